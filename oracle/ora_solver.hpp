@@ -1,0 +1,388 @@
+// ora_solver.hpp — grid metrics (O2), halo fill (O3), RHS (O6/O7), SSP-RK3 (O8), CFL (O9)
+// of the CPU ORACLE (test infrastructure, not the product).  Straight loops over cells and
+// faces in the paper's notation; each face flux is computed once and used by both neighbours
+// (Eq. 6).  OpenMP only over independent cells/faces: bit-deterministic.
+#pragma once
+#include <vector>
+#include <cstring>
+#include <limits>
+#include "ora.h"
+#include "ora_core.hpp"
+
+namespace ora {
+
+constexpr int NH = 3;  // halo layers (WENO5 needs 3)
+
+struct Config {
+  int n[3];                       // interior cells nx, ny, nz
+  int P[3];                       // padded sizes n+6
+  std::vector<double> xf[3];      // face coordinates (n+1)
+  std::vector<double> dl[3];      // padded cell widths  (index p = i+3)
+  std::vector<double> xc[3];      // padded cell centres
+  std::vector<double> Xc[3];      // centre metric X_xi^c at padded index (valid for interior)
+  std::vector<double> Xf[3];      // face metric X_xi^f at face "p" = face on the high side of padded cell p
+  double gamma, Rgas, Pr;
+  ora_mu_law mu;
+  ora_bc bc;
+  std::vector<double> dirichlet[6];
+  double g[3];
+  bool viscous;
+};
+
+inline bool axis_periodic(const Config& c, int a) { return c.bc.face[2 * a].type == ORA_BC_PERIODIC; }
+
+// O2: widths, centres, halo geometry (periodic copy or mirror), index-space metrics.
+inline void build_metrics(Config& c) {
+  for (int a = 0; a < 3; ++a) {
+    int N = c.n[a], P = N + 2 * NH;
+    c.P[a] = P;
+    c.dl[a].assign(P, 0.0); c.xc[a].assign(P, 0.0); c.Xc[a].assign(P, 0.0); c.Xf[a].assign(P, 0.0);
+    const std::vector<double>& xf = c.xf[a];
+    for (int i = 0; i < N; ++i) {
+      c.dl[a][i + NH] = xf[i + 1] - xf[i];
+      c.xc[a][i + NH] = 0.5 * (xf[i] + xf[i + 1]);
+    }
+    bool per = axis_periodic(c, a);
+    for (int m = 1; m <= NH; ++m) {
+      // low side ghost -m, high side ghost N-1+m
+      c.dl[a][NH - m] = per ? c.dl[a][NH + N - m] : c.dl[a][NH + m - 1];
+      c.dl[a][NH + N - 1 + m] = per ? c.dl[a][NH + m - 1] : c.dl[a][NH + N - m];
+    }
+    double edge = xf[0];
+    for (int m = 1; m <= NH; ++m) {
+      double w = c.dl[a][NH - m];
+      c.xc[a][NH - m] = edge - 0.5 * w;
+      edge -= w;
+    }
+    edge = xf[N];
+    for (int m = 1; m <= NH; ++m) {
+      double w = c.dl[a][NH + N - 1 + m];
+      c.xc[a][NH + N - 1 + m] = edge + 0.5 * w;
+      edge += w;
+    }
+    const std::vector<double>& x = c.xc[a];
+    for (int i = 0; i < N; ++i) {
+      int p = i + NH;
+      c.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
+    }
+    for (int i = -1; i <= N - 1; ++i) {  // face i+1/2
+      int p = i + NH;
+      c.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
+    }
+  }
+}
+
+template <class R>
+struct Field {  // view of U[5][Pz][Py][Px]
+  R* d; int Px, Py, Pz; size_t plane, vol;
+  Field(R* p, const Config& c) : d(p), Px(c.P[0]), Py(c.P[1]), Pz(c.P[2]) {
+    plane = (size_t)Px * Py; vol = plane * Pz;
+  }
+  // padded indices
+  inline R& at(int q, int pi, int pj, int pk) const {
+    return d[(size_t)q * vol + (size_t)pk * plane + (size_t)pj * Px + pi];
+  }
+  // interior-based indices (may be -3..n+2)
+  inline R& operator()(int q, int i, int j, int k) const { return at(q, i + NH, j + NH, k + NH); }
+};
+
+// ---------------------------------------------------------------- O3 halo fill
+// Order: x faces for interior (j,k); y faces for interior k and all padded i; z faces for
+// all padded (i,j).  Ghost index g = -m, mirror index r = m-1 (m = 1..3); high side symmetric.
+template <class R>
+void fill_halo(const Config& c, R* Uptr) {
+  Field<R> U(Uptr, c);
+  const R gamma = R(c.gamma), Rgas = R(c.Rgas);
+  for (int a = 0; a < 3; ++a) {
+    int t1a, t2a;  // tangential axes used for (t1, t2): x-face (y,z), y-face (x,z), z-face (x,y)
+    if (a == 0) { t1a = 1; t2a = 2; } else if (a == 1) { t1a = 0; t2a = 2; } else { t1a = 0; t2a = 1; }
+    // ranges of the two tangential padded indices
+    int lo[3] = {0, 0, 0}, hi[3] = {c.P[0], c.P[1], c.P[2]};
+    if (a == 0) { lo[1] = NH; hi[1] = NH + c.n[1]; lo[2] = NH; hi[2] = NH + c.n[2]; }
+    if (a == 1) { lo[2] = NH; hi[2] = NH + c.n[2]; }
+    int N = c.n[a];
+    for (int side = 0; side < 2; ++side) {
+      const ora_bc_face& f = c.bc.face[2 * a + side];
+      const std::vector<double>& dir = c.dirichlet[2 * a + side];
+#pragma omp parallel for collapse(2) schedule(static)
+      for (int p2 = lo[t2a]; p2 < hi[t2a]; ++p2)
+        for (int p1 = lo[t1a]; p1 < hi[t1a]; ++p1)
+          for (int m = 1; m <= NH; ++m) {
+            int g = side == 0 ? -m : N - 1 + m;          // ghost (interior-based)
+            int r = side == 0 ? m - 1 : N - m;           // mirror
+            int src;                                      // source cell for copies
+            int idx[3], ids[3];
+            idx[a] = g + NH; idx[t1a] = p1; idx[t2a] = p2;
+            ids[t1a] = p1; ids[t2a] = p2;
+            if (f.type == ORA_BC_PERIODIC) {
+              src = side == 0 ? N - m : m - 1;
+              ids[a] = src + NH;
+              for (int q = 0; q < 5; ++q) U.at(q, idx[0], idx[1], idx[2]) = U.at(q, ids[0], ids[1], ids[2]);
+            } else if (f.type == ORA_BC_ZEROGRAD) {
+              src = side == 0 ? 0 : N - 1;
+              ids[a] = src + NH;
+              for (int q = 0; q < 5; ++q) U.at(q, idx[0], idx[1], idx[2]) = U.at(q, ids[0], ids[1], ids[2]);
+            } else if (f.type == ORA_BC_DIRICHLET) {
+              // table prim[5][n_t2][n_t1] over interior tangential sizes; padded indices clamp
+              int n1 = c.n[t1a], n2 = c.n[t2a];
+              int c1 = std::min(std::max(p1 - NH, 0), n1 - 1), c2 = std::min(std::max(p2 - NH, 0), n2 - 1);
+              R W[5], Uc[5];
+              for (int q = 0; q < 5; ++q) W[q] = R(dir[((size_t)q * n2 + c2) * n1 + c1]);
+              prim_to_cons(gamma, W, Uc);
+              for (int q = 0; q < 5; ++q) U.at(q, idx[0], idx[1], idx[2]) = Uc[q];
+            } else {  // walls
+              ids[a] = r + NH;
+              R Ur[5], Wr[5];
+              for (int q = 0; q < 5; ++q) Ur[q] = U.at(q, ids[0], ids[1], ids[2]);
+              cons_to_prim(gamma, Ur, Wr);
+              R uw[3] = {R(f.u_wall[0]), R(f.u_wall[1]), R(f.u_wall[2])};
+              if (f.dist.enabled) {
+                double t1 = c.xc[t1a][p1];  // ghost cell's own tangential centre
+                if (t1 >= f.dist.t1_lo && t1 <= f.dist.t1_hi) {
+                  // Eq. 8: wall-normal wall velocity A sin(2 pi kappa t1)
+                  double vw = f.dist.A * std::sin(2.0 * M_PI * f.dist.kappa * t1);
+                  uw[a] = uw[a] + R(vw);
+                }
+              }
+              R Wg[5];
+              for (int d = 0; d < 3; ++d) Wg[1 + d] = R(2) * uw[d] - Wr[1 + d];
+              R pg = Wr[4];
+              R Tr = Wr[4] / (Wr[0] * Rgas), Tg;
+              if (f.type == ORA_BC_WALL_ISOTHERMAL) {
+                R Tw = R(f.T_wall);
+                Tg = R(2) * Tw - Tr;
+                if (Tg <= R(0.05) * Tw) Tg = R(0.05) * Tw;
+              } else {
+                Tg = Tr;
+              }
+              Wg[0] = pg / (Rgas * Tg);
+              Wg[4] = pg;
+              R Ug[5];
+              prim_to_cons(gamma, Wg, Ug);
+              for (int q = 0; q < 5; ++q) U.at(q, idx[0], idx[1], idx[2]) = Ug[q];
+            }
+          }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- primitives over the padded box
+template <class R>
+struct Prim {
+  std::vector<R> W;  // [6][vol]: rho,u,v,w,p,T
+  size_t vol, plane; int Px;
+  inline R& at(int q, int pi, int pj, int pk) { return W[(size_t)q * vol + (size_t)pk * plane + (size_t)pj * Px + pi]; }
+};
+
+template <class R>
+void compute_prims(const Config& c, const R* Uptr, Prim<R>& P) {
+  Field<const R> U(Uptr, c);
+  P.vol = U.vol; P.plane = U.plane; P.Px = U.Px;
+  P.W.assign(6 * U.vol, R(0));
+  const R gamma = R(c.gamma), Rgas = R(c.Rgas);
+#pragma omp parallel for schedule(static)
+  for (int pk = 0; pk < c.P[2]; ++pk)
+    for (int pj = 0; pj < c.P[1]; ++pj)
+      for (int pi = 0; pi < c.P[0]; ++pi) {
+        R Uc[5], Wc[5];
+        for (int q = 0; q < 5; ++q) Uc[q] = U.at(q, pi, pj, pk);
+        cons_to_prim(gamma, Uc, Wc);
+        for (int q = 0; q < 5; ++q) P.at(q, pi, pj, pk) = Wc[q];
+        P.at(5, pi, pj, pk) = Wc[4] / (Wc[0] * Rgas);  // T = p/(rho R)
+      }
+}
+
+// ---------------------------------------------------------------- O6 dissipative flux of one face
+// Face on the high side of padded cell (pc[0],pc[1],pc[2]) along direction d.
+// (n,t1,t2) = (d, d+1, d+2) cyclic.  Eq. 4-5, Fourier q = -lambda grad T.
+template <class R>
+void viscous_face(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) {
+  const int n = d, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  auto val = [&](int q, int sn, int st1, int st2) -> R {  // shifted cell value
+    int id[3] = {pc[0], pc[1], pc[2]};
+    id[n] += sn; id[t1] += st1; id[t2] += st2;
+    return P.at(q, id[0], id[1], id[2]);
+  };
+  const int qn = 1 + n, qt1 = 1 + t1, qt2 = 1 + t2, qT = 5;
+  const R Xf = R(c.Xf[n][pc[n]]);
+  const R Xc1 = R(c.Xc[t1][pc[t1]]), Xc2 = R(c.Xc[t2][pc[t2]]);
+  // normal derivatives D^f and face values I^f
+  R dn_un = d_face(val(qn, -1, 0, 0), val(qn, 0, 0, 0), val(qn, 1, 0, 0), val(qn, 2, 0, 0), Xf);
+  R dn_ut1 = d_face(val(qt1, -1, 0, 0), val(qt1, 0, 0, 0), val(qt1, 1, 0, 0), val(qt1, 2, 0, 0), Xf);
+  R dn_ut2 = d_face(val(qt2, -1, 0, 0), val(qt2, 0, 0, 0), val(qt2, 1, 0, 0), val(qt2, 2, 0, 0), Xf);
+  R dn_T = d_face(val(qT, -1, 0, 0), val(qT, 0, 0, 0), val(qT, 1, 0, 0), val(qT, 2, 0, 0), Xf);
+  R un_f = i_face(val(qn, -1, 0, 0), val(qn, 0, 0, 0), val(qn, 1, 0, 0), val(qn, 2, 0, 0));
+  R ut1_f = i_face(val(qt1, -1, 0, 0), val(qt1, 0, 0, 0), val(qt1, 1, 0, 0), val(qt1, 2, 0, 0));
+  R ut2_f = i_face(val(qt2, -1, 0, 0), val(qt2, 0, 0, 0), val(qt2, 1, 0, 0), val(qt2, 2, 0, 0));
+  R T_f = i_face(val(qT, -1, 0, 0), val(qT, 0, 0, 0), val(qT, 1, 0, 0), val(qT, 2, 0, 0));
+  // transverse derivatives: I^f over the centre derivatives D^c at cells -1..2 along n
+  R g1n[4], g11[4], g2n[4], g22[4];
+  for (int m = -1; m <= 2; ++m) {
+    g1n[m + 1] = d_centre(val(qn, m, -2, 0), val(qn, m, -1, 0), val(qn, m, 1, 0), val(qn, m, 2, 0), Xc1);
+    g11[m + 1] = d_centre(val(qt1, m, -2, 0), val(qt1, m, -1, 0), val(qt1, m, 1, 0), val(qt1, m, 2, 0), Xc1);
+    g2n[m + 1] = d_centre(val(qn, m, 0, -2), val(qn, m, 0, -1), val(qn, m, 0, 1), val(qn, m, 0, 2), Xc2);
+    g22[m + 1] = d_centre(val(qt2, m, 0, -2), val(qt2, m, 0, -1), val(qt2, m, 0, 1), val(qt2, m, 0, 2), Xc2);
+  }
+  R dt1_un = i_face(g1n[0], g1n[1], g1n[2], g1n[3]);
+  R dt1_ut1 = i_face(g11[0], g11[1], g11[2], g11[3]);
+  R dt2_un = i_face(g2n[0], g2n[1], g2n[2], g2n[3]);
+  R dt2_ut2 = i_face(g22[0], g22[1], g22[2], g22[3]);
+  R mu = viscosity(c.mu.sutherland, R(c.mu.mu_ref), R(c.mu.T_ref), R(c.mu.S), T_f);
+  R cp = R(c.gamma * c.Rgas / (c.gamma - 1.0));
+  R lambda = mu * cp / R(c.Pr);
+  R div = dn_un + dt1_ut1 + dt2_ut2;
+  R tau_nn = mu * (R(2) * dn_un - R(2.0 / 3.0) * div);
+  R tau_nt1 = mu * (dt1_un + dn_ut1);
+  R tau_nt2 = mu * (dt2_un + dn_ut2);
+  Fd[0] = R(0);
+  Fd[qn] = tau_nn; Fd[qt1] = tau_nt1; Fd[qt2] = tau_nt2;
+  Fd[4] = un_f * tau_nn + ut1_f * tau_nt1 + ut2_f * tau_nt2 + lambda * dn_T;
+}
+
+// ---------------------------------------------------------------- O7 RHS of Eq. 6
+template <class R>
+void rhs(const Config& c, const R* Uptr, R* Rptr, bool inviscid, bool viscous, bool source) {
+  Prim<R> P;
+  compute_prims(c, Uptr, P);
+  Field<R> Rf(Rptr, c);
+  const R gamma = R(c.gamma);
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int d = 0; d < 3; ++d) {
+    // faces along d: face index f = -1..n_d-1 (high side of cell f); other indices interior
+    int nf[3] = {nx, ny, nz};
+    nf[d] += 1;
+    std::vector<R> F((size_t)5 * nf[0] * nf[1] * nf[2]);
+    auto Fat = [&](int q, int a, int b, int cc) -> R& {
+      return F[(((size_t)q * nf[2] + cc) * nf[1] + b) * nf[0] + a];
+    };
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int fk = 0; fk < nf[2]; ++fk)
+      for (int fj = 0; fj < nf[1]; ++fj)
+        for (int fi = 0; fi < nf[0]; ++fi) {
+          int cell[3] = {fi, fj, fk};
+          cell[d] -= 1;  // interior-based index of the cell on the low side of the face
+          int pc[3] = {cell[0] + NH, cell[1] + NH, cell[2] + NH};
+          R Fc[5] = {R(0), R(0), R(0), R(0), R(0)}, Fd[5] = {R(0), R(0), R(0), R(0), R(0)};
+          if (inviscid) {
+            R WL[5], WR[5];
+            for (int q = 0; q < 5; ++q) {
+              R s[6];
+              for (int m = -2; m <= 3; ++m) {
+                int id[3] = {pc[0], pc[1], pc[2]};
+                id[d] += m;
+                s[m + 2] = P.at(q, id[0], id[1], id[2]);
+              }
+              WL[q] = weno5(s[0], s[1], s[2], s[3], s[4]);  // q_{i-2..i+2}
+              WR[q] = weno5(s[5], s[4], s[3], s[2], s[1]);  // q_{i+3..i-1}
+            }
+            hllc(d, gamma, WL, WR, Fc);
+          }
+          if (viscous && c.viscous) viscous_face(c, P, d, pc, Fd);
+          for (int q = 0; q < 5; ++q) Fat(q, fi, fj, fk) = Fc[q] - Fd[q];
+        }
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          int hi[3] = {i, j, k};
+          hi[d] += 1;
+          int cidx[3] = {i, j, k};
+          R delta = R(c.dl[d][cidx[d] + NH]);  // Delta x_{i,j,k} of Eq. 6
+          for (int q = 0; q < 5; ++q) {
+            R dF = (Fat(q, hi[0], hi[1], hi[2]) - Fat(q, i, j, k)) / delta;
+            if (d == 0) Rf(q, i, j, k) = -dF;
+            else Rf(q, i, j, k) = Rf(q, i, j, k) - dF;
+          }
+        }
+  }
+  if (source) {
+    const R g[3] = {R(c.g[0]), R(c.g[1]), R(c.g[2])};
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          R rho = P.at(0, i + NH, j + NH, k + NH), u = P.at(1, i + NH, j + NH, k + NH);
+          R v = P.at(2, i + NH, j + NH, k + NH), w = P.at(3, i + NH, j + NH, k + NH);
+          Rf(1, i, j, k) = Rf(1, i, j, k) + rho * g[0];
+          Rf(2, i, j, k) = Rf(2, i, j, k) + rho * g[1];
+          Rf(3, i, j, k) = Rf(3, i, j, k) + rho * g[2];
+          Rf(4, i, j, k) = Rf(4, i, j, k) + rho * (u * g[0] + v * g[1] + w * g[2]);
+        }
+  }
+}
+
+// ---------------------------------------------------------------- O8 SSP-RK3 (Shu-Osher)
+//   U1 = U^n + dt L(U^n);  U2 = 3/4 U^n + 1/4 (U1 + dt L(U1));  U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
+// with L(U) = R(fill_halo(U)); interior cells only.
+template <class R>
+void rk3_step(const Config& c, R* U, R dt) {
+  size_t ne = (size_t)5 * c.P[0] * c.P[1] * c.P[2];
+  std::vector<R> Rr(ne, R(0)), U1(U, U + ne), U2(ne);
+  Field<R> Un(U, c), F1(U1.data(), c), F2(U2.data(), c), FR(Rr.data(), c);
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  fill_halo(c, U);
+  rhs(c, U, Rr.data(), true, true, true);
+  U1.assign(U, U + ne);
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i)
+        for (int q = 0; q < 5; ++q) F1(q, i, j, k) = Un(q, i, j, k) + dt * FR(q, i, j, k);
+  fill_halo(c, U1.data());
+  rhs(c, U1.data(), Rr.data(), true, true, true);
+  U2 = U1;
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i)
+        for (int q = 0; q < 5; ++q)
+          F2(q, i, j, k) = R(0.75) * Un(q, i, j, k) + R(0.25) * (F1(q, i, j, k) + dt * FR(q, i, j, k));
+  fill_halo(c, U2.data());
+  rhs(c, U2.data(), Rr.data(), true, true, true);
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i)
+        for (int q = 0; q < 5; ++q)
+          Un(q, i, j, k) = R(1.0 / 3.0) * Un(q, i, j, k) + R(2.0 / 3.0) * (F2(q, i, j, k) + dt * FR(q, i, j, k));
+}
+
+// ---------------------------------------------------------------- O9 CFL time step
+//   dt_conv = min_cells min_d Delta_d/(|u_d|+c);  dt_visc = 3/14 min Dmin^2 rho/mu;
+//   dt_heat = 1/10 min Dmin^2 rho Pr/mu;  dt = cfl*min(...)   (mu_ref = 0: convective only)
+template <class R>
+int cfl_dt(const Config& c, const R* Uptr, double cfl, double* dt_out) {
+  Field<const R> U(Uptr, c);
+  const R gamma = R(c.gamma), Rgas = R(c.Rgas);
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  R inf = std::numeric_limits<R>::infinity();
+  R dconv = inf, dvisc = inf, dheat = inf;
+  bool bad = false;
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        R Uc[5], W[5];
+        for (int q = 0; q < 5; ++q) Uc[q] = U(q, i, j, k);
+        cons_to_prim(gamma, Uc, W);
+        bool ok = true;
+        for (int q = 0; q < 5; ++q) ok = ok && std::isfinite(Uc[q]);
+        if (!ok || !(W[0] > R(0)) || !(W[4] > R(0))) { bad = true; continue; }
+        R cs = s_sqrt(gamma * W[4] / W[0]);
+        R dl[3] = {R(c.dl[0][i + NH]), R(c.dl[1][j + NH]), R(c.dl[2][k + NH])};
+        for (int d = 0; d < 3; ++d) dconv = s_min(dconv, dl[d] / (s_abs(W[1 + d]) + cs));
+        if (c.viscous) {
+          R dmin = s_min(dl[0], s_min(dl[1], dl[2]));
+          R T = W[4] / (W[0] * Rgas);
+          R mu = viscosity(c.mu.sutherland, R(c.mu.mu_ref), R(c.mu.T_ref), R(c.mu.S), T);
+          dvisc = s_min(dvisc, dmin * dmin * W[0] / mu);
+          dheat = s_min(dheat, dmin * dmin * W[0] * R(c.Pr) / mu);
+        }
+      }
+  if (bad) { *dt_out = std::numeric_limits<double>::quiet_NaN(); return ORA_ENOTFINITE; }
+  R dt = dconv;
+  if (c.viscous) dt = s_min(dt, s_min(R(3.0 / 14.0) * dvisc, R(1.0 / 10.0) * dheat));
+  *dt_out = cfl * (double)dt;
+  return ORA_OK;
+}
+
+}  // namespace ora
