@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the hot path (BASELINE.json metric: cell-updates/s per RK3 step, fp64,
+1 B200, and fraction of the fp64 roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size n] [--dtype f64|f32] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: jf_rk3_step = 3 x (halo fill, centre gradients, x/y/z
+sweeps with WENO5 + HLLC + viscous flux, divergence, RK3 stage) on the Taylor-Green input of
+BASELINE.json configs[4] (default 256^3 fp64: the size north_star's target is quoted at; the state is
+719 MB, i.e. larger than the 126 MB L2, so every step streams from HBM — no L2 flush needed).
+Prints ONE JSON line (rank 0).  N > 1: independent replicas, one per GPU (the path has no exchange
+step on one GPU), barrier + max-over-ranks timing, value = all cells / time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s per RK3 step"
+UNIT = "cell-updates/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--size", type=int, default=256, help="n of the n^3 Taylor-Green box")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-size", type=int, default=96, help="n^3 sample the reference arm steps")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------- flop model (oracle count)
+def flop_model(n):
+    """Algorithmic flops per interior cell from oracle/flop_model.json (written by
+    oracle/count_flops.py from the oracle's counting build): step, one RHS, prim, grad."""
+    with open(os.path.join(ROOT, "oracle", "flop_model.json")) as f:
+        m = json.load(f)
+    x = 1.0 / n
+    ev = lambda key: sum(c * x ** k for k, c in enumerate(m[key][3]))
+    return {k: ev(k) for k in ("step", "rhs", "prim", "grad")}
+
+
+# ---------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            p = [s.strip() for s in ln.split(",")]
+            if len(p) < 8:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2])); pw.append(float(p[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[4:8]):
+                if v == "Active":
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------- reference arm = the oracle
+def oracle_throughput(n, steps, warmup):
+    """The oracle as it stands (oracle/libora.so, -O2 -ffp-contract=off -fopenmp) on the host cores."""
+    from oracle import ora
+    from paper_2406_19494_b200 import cases
+    case = cases.tgv(n)
+    o = ora.Oracle(case)
+    U = o.state()
+    for _ in range(warmup):
+        o.rk3_step(U, case.dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.rk3_step(U, case.dt)
+    dt = time.perf_counter() - t0
+    return case.cells * steps / dt, dt, os.cpu_count()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    val, secs, cores = oracle_throughput(args.ref_size, args.steps, args.warmup)
+    sample = f"tgv {args.ref_size}^3 fp64, {args.steps} RK3 steps after {args.warmup} warm-up (same physics as the GPU arm's {args.size}^3 box)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"tgv{args.size} fp64 (BASELINE.json configs[4])", "reference": "CPU oracle (oracle/), host cores",
+                       "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2406_19494_b200 import binding as jf, cases
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — libjf has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n, K, W = args.size, args.steps, max(args.warmup, 3)
+    case = cases.tgv(n)
+    solver = jf.Solver(case, args.dtype, device=str(dev))
+    esz = 8 if args.dtype == "f64" else 4
+    U = solver.state()
+    dt = case.dt
+    state_bytes = U.numel() * esz
+
+    # --- device-resident throughput: inputs in HBM, K steps between two events
+    for _ in range(W):
+        solver.jf_rk3_step(U, dt)
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    solver.jf_diag_kernel_times()                      # reset
+    solver.jf_diag_timing(True)
+    l0 = solver.jf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        solver.jf_rk3_step(U, dt)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = solver.jf_launch_count() - l0
+    ktimes = solver.jf_diag_kernel_times()
+    solver.jf_diag_timing(False)
+    clk = clocks.stop()
+    finite = bool(torch.isfinite(U).all().item())
+
+    # --- end to end: host buffers, H2D of the input and D2H of the result inside every step
+    e2e = None
+    if not args.no_e2e:
+        host_in = torch.empty(U.shape, dtype=U.dtype, pin_memory=True)
+        host_in.copy_(torch.as_tensor(case.U0, dtype=U.dtype))
+        host_out = torch.empty(U.shape, dtype=U.dtype, pin_memory=True)
+        Ke = K
+        for _ in range(2):
+            U.copy_(host_in, non_blocking=True); solver.jf_rk3_step(U, dt); host_out.copy_(U, non_blocking=True)
+        barrier()
+        t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for _ in range(Ke):
+            U.copy_(host_in, non_blocking=True)
+            solver.jf_rk3_step(U, dt)
+            host_out.copy_(U, non_blocking=True)
+        t1.record()
+        barrier()
+        ms_e2e = t0.elapsed_time(t1)
+        e2e = (ms_e2e, Ke)
+
+    # --- max over ranks
+    if world > 1:
+        t = torch.tensor([ms, e2e[0] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0]); e2e = (float(t[1]), e2e[1]) if e2e else None
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cells = case.cells
+    value = world * cells * K / (ms * 1e-3)
+    fm = flop_model(n)
+    # roofline of the dominant kernel (bound: plain FP64/FP32 ALUs; nothing here is a contraction)
+    peak_flops, _ = jf.jf_diag_alu_peak(args.dtype, 4096)
+    sweep_flops = (fm["rhs"] - fm["prim"] - fm["grad"]) / 3.0           # one direction: WENO5+HLLC+viscous face+divergence
+    rk_flops = (fm["step"] - 3.0 * fm["rhs"]) / 3.0                    # stage update
+    alg = {"sweep_x_kernel": sweep_flops + fm["prim"] / 3.0, "sweep_yz_kernel<y>": sweep_flops + fm["prim"] / 3.0,
+           "sweep_yz_kernel<z>+rk": sweep_flops + fm["prim"] / 3.0 + rk_flops, "gradient_kernel": fm["grad"]}
+    dom = max((k for k in ktimes if ktimes[k][1] > 0), key=lambda k: ktimes[k][0])
+    dom_ms, dom_n = ktimes[dom]
+    dom_flops = alg.get(dom, 0.0) * cells
+    achieved = dom_flops / (dom_ms / dom_n * 1e-3) / 1e12 if dom_n else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"{dom}|{n}|{args.dtype}")
+    peaks = {}
+    ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(ppath):
+        peaks = json.load(open(ppath))
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    t_roof_ms = max(fm["step"] * cells / peak_flops, (320 if args.dtype == "f64" else 160) * cells / (hbm * 1e9)) * 1e3
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"tgv{n} {'fp64' if args.dtype == 'f64' else 'fp32'} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)",
+                   "cells": cells, "state_bytes": state_bytes, "l2": "inputs larger than L2 (no flush)" if state_bytes > 126e6 else "state fits L2",
+                   "parallelism": f"replicas x{world}" if world > 1 else "1 GPU", "finite": finite},
+        "clocks": clk,
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
+                     "frac": achieved / (peak_flops / 1e12), "traffic": traffic,
+                     "peak_source": "measured live: jf_diag_alu_peak register-resident FMA loop (DESIGN.md)",
+                     "flops_per_cell_launch": alg.get(dom), "avg_launch_ms": dom_ms / dom_n if dom_n else None},
+        "roofline_step": {"flops_per_cell_step": fm["step"], "t_roof_ms": t_roof_ms, "frac": t_roof_ms / (ms / K),
+                          "hbm_gbs": hbm, "hbm_source": "measured" if peaks else "fallback"},
+        "kernels_ms_per_step": {k: v[0] / K for k, v in ktimes.items() if v[1]},
+    }
+    if e2e:
+        line["e2e"] = {"value": world * cells * e2e[1] / (e2e[0] * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes, "ms_per_step": e2e[0] / e2e[1]}
+    if world == 1 and not args.no_cpu_baseline:
+        # bounded sample: one RK3 step of the SAME input on the host cores (the oracle as it stands)
+        nb = min(n, 256)
+        val, secs, cores = oracle_throughput(nb, 1, 0)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"1 RK3 step of tgv{nb} fp64 ({secs:.1f} s)"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -1,0 +1,144 @@
+/* jf.h — C ABI of libjf: B200-native (sm_100a) finite-volume right-hand side of the 3-D
+ * compressible Navier-Stokes equations on a structured, optionally stretched Cartesian grid,
+ * after arxiv/paper_2406_19494.
+ *
+ * What the calls compute (citations are PAPER.md line numbers):
+ *   state U = [rho, rho u, rho v, rho w, E], E = rho e + 1/2 rho u.u         Eq. 2, :44-46
+ *   dU/dt = R_NSE(U): flux divergence of convective (Eq. 3, :50) minus dissipative (Eq. 4-5,
+ *   :54-62) face fluxes with per-cell widths, plus sources                   Eq. 6, :64-69
+ *   convective face flux: WENO-type reconstruction + approximate Riemann solver (:72) —
+ *   here WENO5-JS on primitive variables + HLLC (:88); dissipative flux: central finite
+ *   differences (:72) — here 4th order, Sutherland viscosity (:108), Fourier heat flux (:62)
+ *   time integration: explicit TVD Runge-Kutta (:72) — here SSP-RK3
+ *   arrays carry Nh = 3 halo cells per side, shape [N+2Nh]^3 (:80); boundary conditions are
+ *   imposed by assigning the halo cells (:100): periodic, zero-gradient, Dirichlet, no-slip wall
+ *   (isothermal / adiabatic) and the paper's "Disturbance Wall" v = A sin(2 pi kappa x)
+ *   (:102-104, Eq. 8 :112), which with A = 0 is exactly the no-slip wall (:104).
+ * Formulas the paper does not print are fixed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - All functions return jf_status (0 = success) unless noted; no exception crosses the ABI.
+ *   - "dev" pointers are DEVICE pointers owned by the caller (e.g. torch tensors); "host"
+ *     pointers are host memory.  The library allocates no device memory for fields: scratch
+ *     is the caller's workspace (jf_workspace_bytes).  Small metric/BC tables are carved out of
+ *     the same workspace.
+ *   - State layout: jf_state_elems() contiguous elements of the solver's dtype,
+ *       index ((q*(nz+6) + k+3)*(ny+6) + j+3)*(nx+6) + i+3,  q in {rho, rho u, rho v, rho w, E},
+ *     x fastest; base address 16-byte aligned (JF_EALIGN otherwise).
+ *   - Every launch goes to the cuda_stream given to jf_create (a cudaStream_t passed as
+ *     void*; NULL = default stream).  Only jf_cfl_dt and jf_diag_* synchronise that stream.
+ *   - One jf_solver per host thread / stream (thread-compatible, not thread-safe).
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with JF_ECUDA.
+ */
+#ifndef JF_H
+#define JF_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct jf_solver jf_solver; /* opaque */
+
+typedef enum {
+  JF_OK = 0, JF_EINVAL = 1, JF_EALIGN = 2, JF_EWORKSPACE = 3, JF_ECUDA = 4, JF_ENOTFINITE = 5
+} jf_status;
+typedef enum { JF_F64 = 0, JF_F32 = 1 } jf_dtype;
+typedef enum {
+  JF_BC_PERIODIC = 0, JF_BC_ZEROGRAD = 1, JF_BC_DIRICHLET = 2,
+  JF_BC_WALL_ISOTHERMAL = 3, JF_BC_WALL_ADIABATIC = 4
+} jf_bc_type;
+
+/* Grid: face coordinates per axis (host pointers, copied by jf_create), strictly increasing.
+ * Stretched meshes (:31, :104) are given through these arrays; Delta x_{i,j,k} of Eq. 6 is
+ * xf[i+1]-xf[i].  Each n >= 4. */
+typedef struct {
+  int nx, ny, nz;
+  const double *xf, *yf, *zf; /* nx+1, ny+1, nz+1 entries */
+} jf_grid;
+
+/* Viscosity law (:108): sutherland != 0: mu = mu_ref (T/T_ref)^1.5 (T_ref+S)/(T+S);
+ * sutherland == 0: mu = mu_ref.  mu_ref == 0 means inviscid (dissipative flux skipped). */
+typedef struct { int sutherland; double mu_ref, T_ref, S; } jf_mu_law;
+
+/* Disturbance ("porous") segment on a wall face, Eq. 8 (:112): wall-normal wall velocity
+ * v_w(t1) = A sin(2 pi kappa t1) added where t1_lo <= t1 <= t1_hi, t1 = the ghost cell's own
+ * centre coordinate along the first tangential axis (x for y and z faces, y for x faces);
+ * positive = along the + axis.  Elsewhere the plain wall. */
+typedef struct { int enabled; double A, kappa, t1_lo, t1_hi; } jf_disturbance;
+
+typedef struct {
+  jf_bc_type type;
+  double T_wall;           /* isothermal walls                                            */
+  double u_wall[3];        /* wall velocity vector (u,v,w); 0 for a wall at rest          */
+  const double *dirichlet; /* JF_BC_DIRICHLET: host array prim[5][n_t2][n_t1] of
+                              (rho,u,v,w,p) over the interior tangential sizes (x faces:
+                              t1=y,t2=z; y faces: t1=x,t2=z; z faces: t1=x,t2=y); copied     */
+  jf_disturbance dist;     /* walls only */
+} jf_bc_face;
+typedef struct { jf_bc_face face[6]; } jf_bc; /* x-, x+, y-, y+, z-, z+; periodic must pair */
+
+/* Bytes of device workspace jf_create needs for this grid and dtype (0 on invalid input). */
+size_t jf_workspace_bytes(const jf_grid *grid, jf_dtype dtype);
+
+/* Create a solver.  Validates: n >= 4, monotone faces, gamma > 1, R_gas > 0, Pr > 0,
+ * mu_ref >= 0, periodic faces paired, Dirichlet pointer non-null, T_wall > 0 on isothermal
+ * walls (else JF_EINVAL, *out = NULL); workspace_dev 256-byte aligned (JF_EALIGN) and at least
+ * jf_workspace_bytes() (JF_EWORKSPACE).  body_accel = constant acceleration g of the source
+ * term S = [0, rho g, rho u.g] (Eq. 1 :39-42), may be NULL (= 0).  Copies the metric and BC
+ * tables to the workspace (synchronous small copies).  The workspace must outlive the solver. */
+jf_status jf_create(jf_solver **out, const jf_grid *grid, jf_dtype dtype, double gamma,
+                    double R_gas, double Pr, const jf_mu_law *mu, const jf_bc *bc,
+                    const double body_accel[3], void *workspace_dev, size_t workspace_bytes,
+                    void *cuda_stream);
+jf_status jf_destroy(jf_solver *s);
+
+/* 5*(nz+6)*(ny+6)*(nx+6) */
+size_t jf_state_elems(const jf_solver *s);
+
+/* Halo / boundary fill (:80, :100-104, Eq. 8), in place, asynchronous.  Order x, y, z; the y
+ * pass runs over all padded i and the z pass over all padded (i,j), which defines every edge
+ * and corner cell. */
+jf_status jf_fill_halo(jf_solver *s, void *U_dev);
+
+/* R = R_NSE(U) of Eq. 6 on interior cells (halo cells of R are left untouched).  The halos of
+ * U must already be filled.  U and R must not alias.  Asynchronous. */
+jf_status jf_rhs(jf_solver *s, const void *U_dev, void *R_dev);
+
+/* One SSP-RK3 step in place: 3 x (halo fill, R_NSE, stage update)
+ *   U1 = U + dt L(U);  U2 = 3/4 U + 1/4 (U1 + dt L(U1));  U <- 1/3 U + 2/3 (U2 + dt L(U2)).
+ * On return the interior of U is U^{n+1}; its halo cells hold the fill of U^n.  Asynchronous. */
+jf_status jf_rk3_step(jf_solver *s, void *U_dev, double dt);
+
+/* CFL time step over interior cells (not in the paper; reading O9):
+ *   dt = cfl * min( min_d Delta_d/(|u_d|+c), 3/14 Dmin^2 rho/mu, 1/10 Dmin^2 rho Pr/mu ).
+ * Writes *dt_host and synchronises the stream.  JF_ENOTFINITE (and *dt_host = NaN) if any
+ * interior cell is non-finite or has rho <= 0 or p <= 0. */
+jf_status jf_cfl_dt(jf_solver *s, const void *U_dev, double cfl, double *dt_host);
+
+/* Last error text of this solver ("" if none); never NULL. */
+const char *jf_last_error(const jf_solver *s);
+
+/* Number of kernel launches issued by this solver since jf_create (for bench accounting). */
+unsigned long long jf_launch_count(const jf_solver *s);
+
+/* Diagnostics (not on the hot path): register-resident FMA loop on the plain FP64 (dtype
+ * JF_F64) or FP32 ALUs; writes the achieved FLOP/s (2 per FMA) to *flops_host.  Used by
+ * bench.py as the measured ALU peak of the roofline.  Synchronises the device. */
+jf_status jf_diag_alu_peak(jf_dtype dtype, int iters, double *flops_host, double *ms_host);
+
+/* Per-kernel device timing (diagnostic).  jf_diag_timing(s, 1) makes every launch of this solver
+ * record a CUDA-event pair on its stream; jf_diag_kernel_times synchronises the stream, writes the
+ * accumulated milliseconds and launch counts per kernel class since the previous call (6 classes:
+ * 0 halo (3 launches per fill), 1 gradient, 2 x sweep, 3 y sweep, 4 z sweep + RK3 stage, 5 CFL)
+ * and resets them.  jf_diag_kernel_name(k) names class k ("" if out of range). */
+jf_status jf_diag_timing(jf_solver *s, int enable);
+jf_status jf_diag_kernel_times(jf_solver *s, double ms[6], unsigned long long launches[6]);
+const char *jf_diag_kernel_name(int k);
+
+/* Library version / build info string (static storage). */
+const char *jf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -10,25 +10,31 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "libora.so")
+# Second build of the SAME sources with FMA contraction allowed: used only to measure how much
+# the oracle's own result moves under a legal change of rounding (tests' sensitivity band).
+LIB_FMA = os.path.join(HERE, "libora_fma.so")
 SOURCES = ["ora_capi.cpp"]
 HEADERS = ["ora.h", "ora_core.hpp", "ora_solver.hpp", "ora_naive.hpp"]
 
 
-def needs_build():
-    if not os.path.exists(LIB):
+def needs_build(lib=LIB):
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(os.path.join(HERE, f)) > t for f in SOURCES + HEADERS + ["build.py"])
 
 
-def build(force=False):
-    if not force and not needs_build():
-        return LIB
-    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-o", LIB] + [os.path.join(HERE, s) for s in SOURCES]
+def build(force=False, variant="ref"):
+    lib = LIB if variant == "ref" else LIB_FMA
+    if not force and not needs_build(lib):
+        return lib
+    fp = ["-ffp-contract=off"] if variant == "ref" else ["-ffp-contract=fast", "-mfma"]
+    cmd = ["g++", "-std=c++17", "-O2"] + fp + ["-fopenmp", "-fPIC", "-shared",
+           "-Wall", "-o", lib] + [os.path.join(HERE, s) for s in SOURCES]
     subprocess.check_call(cmd, cwd=HERE)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv))
+    print(build(force="--force" in sys.argv, variant="fma"))

@@ -72,6 +72,9 @@ int ora_rhs_parts(ora_solver *s, const void *U, void *R, int inviscid, int visco
    counts[0]=add/sub/mul/min/max (1 each), [1]=div, [2]=sqrt, [3]=total. */
 int ora_count_flops_step(ora_solver *s, const void *U, double dt, double counts[4]);
 
+/* same convention; what: 1 = cons->prim over the padded box, 2 = centre gradients, 3 = one RHS */
+int ora_count_flops_part(ora_solver *s, const void *U, int what, double counts[4]);
+
 /* grid metrics (padded arrays of length n+6 for axis a in 0..2): widths and centres */
 int ora_metrics(const ora_solver *s, int axis, double *delta, double *centre);
 

@@ -43,13 +43,14 @@ class BC(C.Structure):
     _fields_ = [("face", BCFace * 6)]
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        path = _build.build()
+def lib(variant="ref"):
+    """variant "ref": the oracle (-ffp-contract=off).  "fma": same sources with FMA contraction,
+    only for measuring the oracle's own round-off sensitivity."""
+    if variant not in _libs:
+        path = _build.build(variant=variant)
         L = C.CDLL(path)
         L.ora_create.restype = C.c_int
         L.ora_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(Grid), C.c_int, C.c_double, C.c_double,
@@ -66,6 +67,7 @@ def lib():
         L.ora_rk3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
         L.ora_cfl_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_double, c_double_p]
         L.ora_count_flops_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double, c_double_p]
+        L.ora_count_flops_part.argtypes = [C.c_void_p, C.c_void_p, C.c_int, c_double_p]
         L.ora_metrics.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p]
         L.ora_weno5.argtypes = [c_double_p]
         L.ora_weno5.restype = C.c_double
@@ -88,8 +90,8 @@ def lib():
         L.ora_if.argtypes = [c_double_p]
         L.ora_if.restype = C.c_double
         L.ora_viscous_face.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, c_double_p]
-        _lib = L
-    return _lib
+        _libs[variant] = L
+    return _libs[variant]
 
 
 def _dp(a):
@@ -106,8 +108,9 @@ def _arr(x, n=None):
 class Oracle:
     """The five calls of the oracle on host numpy arrays, built from a cases.Case."""
 
-    def __init__(self, case, dtype="f64"):
+    def __init__(self, case, dtype="f64", variant="ref"):
         self.case = case
+        self.L = lib(variant)
         self.np_dtype = np.float64 if dtype == "f64" else np.float32
         self._keep = []
         nx, ny, nz = case.n
@@ -130,7 +133,7 @@ class Oracle:
                 b.dist = Disturbance(1, fb.dist["A"], fb.dist["kappa"], fb.dist["t1_lo"], fb.dist["t1_hi"])
         ga = _arr(case.body_accel, 3)
         h = C.c_void_p()
-        st = lib().ora_create(C.byref(h), C.byref(g), 0 if dtype == "f64" else 1, case.gamma, case.R_gas,
+        st = self.L.ora_create(C.byref(h), C.byref(g), 0 if dtype == "f64" else 1, case.gamma, case.R_gas,
                               case.Pr, C.byref(mu), C.byref(bc), _dp(ga))
         if st != 0:
             raise ValueError(f"ora_create failed with status {st}")
@@ -138,8 +141,8 @@ class Oracle:
         self.shape = (5, nz + 6, ny + 6, nx + 6)
 
     def __del__(self):
-        if getattr(self, "h", None) and _lib is not None:
-            _lib.ora_destroy(self.h)
+        if getattr(self, "h", None) and getattr(self, "L", None) is not None:
+            self.L.ora_destroy(self.h)
             self.h = None
 
     def state(self, U0=None):
@@ -152,55 +155,61 @@ class Oracle:
 
     def fill_halo(self, U):
         self._chk(U)
-        assert lib().ora_fill_halo(self.h, U.ctypes.data) == 0
+        assert self.L.ora_fill_halo(self.h, U.ctypes.data) == 0
         return U
 
     def rhs(self, U, naive=False, parts=None):
         self._chk(U)
         R = np.zeros_like(U)
         if naive:
-            st = lib().ora_rhs_naive(self.h, U.ctypes.data, R.ctypes.data)
+            st = self.L.ora_rhs_naive(self.h, U.ctypes.data, R.ctypes.data)
         elif parts is not None:
-            st = lib().ora_rhs_parts(self.h, U.ctypes.data, R.ctypes.data, *[int(p) for p in parts])
+            st = self.L.ora_rhs_parts(self.h, U.ctypes.data, R.ctypes.data, *[int(p) for p in parts])
         else:
-            st = lib().ora_rhs(self.h, U.ctypes.data, R.ctypes.data)
+            st = self.L.ora_rhs(self.h, U.ctypes.data, R.ctypes.data)
         assert st == 0
         return R
 
     def rk3_step(self, U, dt):
         self._chk(U)
-        assert lib().ora_rk3_step(self.h, U.ctypes.data, float(dt)) == 0
+        assert self.L.ora_rk3_step(self.h, U.ctypes.data, float(dt)) == 0
         return U
 
     def cfl_dt(self, U, cfl):
         self._chk(U)
         dt = C.c_double()
-        st = lib().ora_cfl_dt(self.h, U.ctypes.data, float(cfl), C.byref(dt))
+        st = self.L.ora_cfl_dt(self.h, U.ctypes.data, float(cfl), C.byref(dt))
         return st, dt.value
 
     def count_flops_step(self, U, dt):
         self._chk(U)
         out = np.zeros(4)
-        assert lib().ora_count_flops_step(self.h, U.ctypes.data, float(dt), _dp(out)) == 0
+        assert self.L.ora_count_flops_step(self.h, U.ctypes.data, float(dt), _dp(out)) == 0
+        return out
+
+    def count_flops_part(self, U, what):
+        self._chk(U)
+        out = np.zeros(4)
+        assert self.L.ora_count_flops_part(self.h, U.ctypes.data, int(what), _dp(out)) == 0
         return out
 
     def metrics(self, axis):
         n = self.case.n[axis] + 6
         d, c = np.zeros(n), np.zeros(n)
-        assert lib().ora_metrics(self.h, axis, _dp(d), _dp(c)) == 0
+        assert self.L.ora_metrics(self.h, axis, _dp(d), _dp(c)) == 0
         return d, c
 
     def viscous_face(self, U, d, i, j, k):
         self._chk(U)
         F = np.zeros(5)
-        assert lib().ora_viscous_face(self.h, U.ctypes.data, d, i, j, k, _dp(F)) == 0
+        assert self.L.ora_viscous_face(self.h, U.ctypes.data, d, i, j, k, _dp(F)) == 0
         return F
 
 
-def run_case(case, dtype="f64", n_steps=None, log=None):
+def run_case(case, dtype="f64", n_steps=None, log=None, variant="ref"):
     """Advance a case with the oracle exactly as the drivers do: fixed dt x n_steps, or CFL steps
     (clipped to t_end when given).  Returns (U, list of dt)."""
-    o = Oracle(case, dtype)
+    o = Oracle(case, dtype, variant)
     U = o.state()
     dts, t = [], 0.0
     n = n_steps if n_steps is not None else case.n_steps

@@ -127,6 +127,36 @@ int ora_count_flops_step(ora_solver* s, const void* U, double dt, double counts[
   return ORA_OK;
 }
 
+int ora_count_flops_part(ora_solver* s, const void* U, int what, double counts[4]) {
+  // what: 1 = cons->prim over the padded box, 2 = centre gradients, 3 = one full RHS (Eq. 6)
+  if (!s || !U || !counts || s->dtype != ORA_F64 || what < 1 || what > 3) return ORA_EINVAL;
+  size_t ne = ora_state_elems(s);
+  std::vector<ora::Cnt> Uc(ne), Rc(ne);
+  const double* Ud = (const double*)U;
+  for (size_t i = 0; i < ne; ++i) Uc[i].v = Ud[i];
+  int saved = 1;
+#ifdef _OPENMP
+  saved = omp_get_max_threads();
+  omp_set_num_threads(1);
+#endif
+  ora::Prim<ora::Cnt> P;
+  ora::Cnt::n_basic = ora::Cnt::n_div = ora::Cnt::n_sqrt = 0;
+  if (what == 1) ora::compute_prims<ora::Cnt>(s->c, Uc.data(), P);
+  if (what == 2) {
+    ora::compute_prims<ora::Cnt>(s->c, Uc.data(), P);
+    ora::Cnt::n_basic = ora::Cnt::n_div = ora::Cnt::n_sqrt = 0;
+    ora::compute_gradients<ora::Cnt>(s->c, P);
+  }
+  if (what == 3) ora::rhs<ora::Cnt>(s->c, Uc.data(), Rc.data(), true, true, true);
+#ifdef _OPENMP
+  omp_set_num_threads(saved);
+#endif
+  (void)saved;
+  counts[0] = ora::Cnt::n_basic; counts[1] = ora::Cnt::n_div; counts[2] = ora::Cnt::n_sqrt;
+  counts[3] = counts[0] + counts[1] + counts[2];
+  return ORA_OK;
+}
+
 int ora_metrics(const ora_solver* s, int axis, double* delta, double* centre) {
   if (!s || axis < 0 || axis > 2) return ORA_EINVAL;
   for (int p = 0; p < s->c.P[axis]; ++p) {
@@ -157,6 +187,7 @@ int ora_viscous_face(ora_solver* s, const void* U, int dir, int i, int j, int k,
   if (!s || !U || s->dtype != ORA_F64 || dir < 0 || dir > 2) return ORA_EINVAL;
   ora::Prim<double> P;
   ora::compute_prims<double>(s->c, (const double*)U, P);
+  ora::compute_gradients<double>(s->c, P);
   int pc[3] = {i + ora::NH, j + ora::NH, k + ora::NH};
   ora::viscous_face<double>(s->c, P, dir, pc, Fd);
   return ORA_OK;

@@ -170,8 +170,12 @@ void fill_halo(const Config& c, R* Uptr) {
 template <class R>
 struct Prim {
   std::vector<R> W;  // [6][vol]: rho,u,v,w,p,T
+  std::vector<R> G;  // [9][vol]: centre derivatives D^c_a u_b at index 3*a+b (filled when viscous)
   size_t vol, plane; int Px;
   inline R& at(int q, int pi, int pj, int pk) { return W[(size_t)q * vol + (size_t)pk * plane + (size_t)pj * Px + pi]; }
+  inline R& grad(int a, int b, int pi, int pj, int pk) {
+    return G[(size_t)(3 * a + b) * vol + (size_t)pk * plane + (size_t)pj * Px + pi];
+  }
 };
 
 template <class R>
@@ -192,6 +196,33 @@ void compute_prims(const Config& c, const R* Uptr, Prim<R>& P) {
       }
 }
 
+// O6: centre derivatives D^c_a u_b of the three velocity components along each axis a, at every
+// cell whose index along a is interior (the other two indices range over the padded box).
+template <class R>
+void compute_gradients(const Config& c, Prim<R>& P) {
+  P.G.assign(9 * P.vol, R(0));
+  for (int a = 0; a < 3; ++a) {
+    int lo[3] = {0, 0, 0}, hi[3] = {c.P[0], c.P[1], c.P[2]};
+    lo[a] = NH; hi[a] = NH + c.n[a];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int pk = lo[2]; pk < hi[2]; ++pk)
+      for (int pj = lo[1]; pj < hi[1]; ++pj)
+        for (int pi = lo[0]; pi < hi[0]; ++pi) {
+          int id[3] = {pi, pj, pk};
+          R Xc = R(c.Xc[a][id[a]]);
+          for (int b = 0; b < 3; ++b) {
+            R v[5];
+            for (int m = -2; m <= 2; ++m) {
+              int jd[3] = {pi, pj, pk};
+              jd[a] += m;
+              v[m + 2] = P.at(1 + b, jd[0], jd[1], jd[2]);
+            }
+            P.grad(a, b, pi, pj, pk) = d_centre(v[0], v[1], v[3], v[4], Xc);
+          }
+        }
+  }
+}
+
 // ---------------------------------------------------------------- O6 dissipative flux of one face
 // Face on the high side of padded cell (pc[0],pc[1],pc[2]) along direction d.
 // (n,t1,t2) = (d, d+1, d+2) cyclic.  Eq. 4-5, Fourier q = -lambda grad T.
@@ -205,7 +236,6 @@ void viscous_face(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) 
   };
   const int qn = 1 + n, qt1 = 1 + t1, qt2 = 1 + t2, qT = 5;
   const R Xf = R(c.Xf[n][pc[n]]);
-  const R Xc1 = R(c.Xc[t1][pc[t1]]), Xc2 = R(c.Xc[t2][pc[t2]]);
   // normal derivatives D^f and face values I^f
   R dn_un = d_face(val(qn, -1, 0, 0), val(qn, 0, 0, 0), val(qn, 1, 0, 0), val(qn, 2, 0, 0), Xf);
   R dn_ut1 = d_face(val(qt1, -1, 0, 0), val(qt1, 0, 0, 0), val(qt1, 1, 0, 0), val(qt1, 2, 0, 0), Xf);
@@ -218,10 +248,12 @@ void viscous_face(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) 
   // transverse derivatives: I^f over the centre derivatives D^c at cells -1..2 along n
   R g1n[4], g11[4], g2n[4], g22[4];
   for (int m = -1; m <= 2; ++m) {
-    g1n[m + 1] = d_centre(val(qn, m, -2, 0), val(qn, m, -1, 0), val(qn, m, 1, 0), val(qn, m, 2, 0), Xc1);
-    g11[m + 1] = d_centre(val(qt1, m, -2, 0), val(qt1, m, -1, 0), val(qt1, m, 1, 0), val(qt1, m, 2, 0), Xc1);
-    g2n[m + 1] = d_centre(val(qn, m, 0, -2), val(qn, m, 0, -1), val(qn, m, 0, 1), val(qn, m, 0, 2), Xc2);
-    g22[m + 1] = d_centre(val(qt2, m, 0, -2), val(qt2, m, 0, -1), val(qt2, m, 0, 1), val(qt2, m, 0, 2), Xc2);
+    int id[3] = {pc[0], pc[1], pc[2]};
+    id[n] += m;
+    g1n[m + 1] = P.grad(t1, n, id[0], id[1], id[2]);
+    g11[m + 1] = P.grad(t1, t1, id[0], id[1], id[2]);
+    g2n[m + 1] = P.grad(t2, n, id[0], id[1], id[2]);
+    g22[m + 1] = P.grad(t2, t2, id[0], id[1], id[2]);
   }
   R dt1_un = i_face(g1n[0], g1n[1], g1n[2], g1n[3]);
   R dt1_ut1 = i_face(g11[0], g11[1], g11[2], g11[3]);
@@ -244,6 +276,7 @@ template <class R>
 void rhs(const Config& c, const R* Uptr, R* Rptr, bool inviscid, bool viscous, bool source) {
   Prim<R> P;
   compute_prims(c, Uptr, P);
+  if (viscous && c.viscous) compute_gradients(c, P);
   Field<R> Rf(Rptr, c);
   const R gamma = R(c.gamma);
   const int nx = c.n[0], ny = c.n[1], nz = c.n[2];

@@ -1,0 +1,261 @@
+"""Thin ctypes binding of libjf.so (include/jf.h): same names, argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA
+kernels.  There is no CPU fallback: if libjf.so is missing or no CUDA device is present the
+calls fail loudly.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjf.so")
+
+JF_OK, JF_EINVAL, JF_EALIGN, JF_EWORKSPACE, JF_ECUDA, JF_ENOTFINITE = range(6)
+JF_F64, JF_F32 = 0, 1
+_STATUS = {0: "JF_OK", 1: "JF_EINVAL", 2: "JF_EALIGN", 3: "JF_EWORKSPACE", 4: "JF_ECUDA", 5: "JF_ENOTFINITE"}
+
+c_double_p = C.POINTER(C.c_double)
+
+
+class jf_grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("xf", c_double_p), ("yf", c_double_p), ("zf", c_double_p)]
+
+
+class jf_mu_law(C.Structure):
+    _fields_ = [("sutherland", C.c_int), ("mu_ref", C.c_double), ("T_ref", C.c_double), ("S", C.c_double)]
+
+
+class jf_disturbance(C.Structure):
+    _fields_ = [("enabled", C.c_int), ("A", C.c_double), ("kappa", C.c_double),
+                ("t1_lo", C.c_double), ("t1_hi", C.c_double)]
+
+
+class jf_bc_face(C.Structure):
+    _fields_ = [("type", C.c_int), ("T_wall", C.c_double), ("u_wall", C.c_double * 3),
+                ("dirichlet", c_double_p), ("dist", jf_disturbance)]
+
+
+class jf_bc(C.Structure):
+    _fields_ = [("face", jf_bc_face * 6)]
+
+
+EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
+           "jf_rk3_step", "jf_cfl_dt", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
+           "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_version"]
+
+_lib = None
+
+
+class JFError(RuntimeError):
+    def __init__(self, status, msg=""):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def lib():
+    """Load libjf.so (raises if it has not been built: no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_2406_19494_b200.build`")
+        L = C.CDLL(LIB_PATH)
+        L.jf_workspace_bytes.restype = C.c_size_t
+        L.jf_workspace_bytes.argtypes = [C.POINTER(jf_grid), C.c_int]
+        L.jf_create.restype = C.c_int
+        L.jf_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(jf_grid), C.c_int, C.c_double, C.c_double,
+                                C.c_double, C.POINTER(jf_mu_law), C.POINTER(jf_bc), c_double_p, C.c_void_p,
+                                C.c_size_t, C.c_void_p]
+        L.jf_destroy.restype = C.c_int
+        L.jf_destroy.argtypes = [C.c_void_p]
+        L.jf_state_elems.restype = C.c_size_t
+        L.jf_state_elems.argtypes = [C.c_void_p]
+        L.jf_fill_halo.restype = C.c_int
+        L.jf_fill_halo.argtypes = [C.c_void_p, C.c_void_p]
+        L.jf_rhs.restype = C.c_int
+        L.jf_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.jf_rk3_step.restype = C.c_int
+        L.jf_rk3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
+        L.jf_cfl_dt.restype = C.c_int
+        L.jf_cfl_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_double, c_double_p]
+        L.jf_last_error.restype = C.c_char_p
+        L.jf_last_error.argtypes = [C.c_void_p]
+        L.jf_launch_count.restype = C.c_ulonglong
+        L.jf_launch_count.argtypes = [C.c_void_p]
+        L.jf_diag_alu_peak.restype = C.c_int
+        L.jf_diag_alu_peak.argtypes = [C.c_int, C.c_int, c_double_p, c_double_p]
+        L.jf_diag_timing.restype = C.c_int
+        L.jf_diag_timing.argtypes = [C.c_void_p, C.c_int]
+        L.jf_diag_kernel_times.restype = C.c_int
+        L.jf_diag_kernel_times.argtypes = [C.c_void_p, c_double_p, C.POINTER(C.c_ulonglong)]
+        L.jf_diag_kernel_name.restype = C.c_char_p
+        L.jf_diag_kernel_name.argtypes = [C.c_int]
+        L.jf_version.restype = C.c_char_p
+        L.jf_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(c_double_p)
+
+
+def _grid_struct(case, keep):
+    nx, ny, nz = case.n
+    arrs = [np.ascontiguousarray(np.asarray(f, dtype=np.float64)) for f in (case.xf, case.yf, case.zf)]
+    keep += arrs
+    return jf_grid(nx, ny, nz, _dp(arrs[0]), _dp(arrs[1]), _dp(arrs[2]))
+
+
+def jf_version():
+    return lib().jf_version().decode()
+
+
+def jf_diag_alu_peak(dtype="f64", iters=4096):
+    fl, ms = C.c_double(), C.c_double()
+    st = lib().jf_diag_alu_peak(JF_F64 if dtype == "f64" else JF_F32, iters, C.byref(fl), C.byref(ms))
+    if st != JF_OK:
+        raise JFError(st, "jf_diag_alu_peak")
+    return fl.value, ms.value
+
+
+class Solver:
+    """jf_solver handle + its device workspace, built from a cases.Case description.
+
+    Methods carry the names of the C calls; tensors are torch CUDA tensors of the solver dtype
+    and shape [5, nz+6, ny+6, nx+6]."""
+
+    def __init__(self, case, dtype="f64", device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise JFError(JF_ECUDA, "no CUDA device: libjf has no CPU fallback")
+        self.torch = torch
+        self.case = case
+        self.device = torch.device(device)
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self._keep = []
+        L = lib()
+        g = _grid_struct(case, self._keep)
+        dt = JF_F64 if dtype == "f64" else JF_F32
+        nbytes = L.jf_workspace_bytes(C.byref(g), dt)
+        if nbytes == 0:
+            raise JFError(JF_EINVAL, "jf_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        ws_ptr = (base + 255) // 256 * 256
+        mu = jf_mu_law(int(case.mu["sutherland"]), case.mu["mu_ref"], case.mu["T_ref"], case.mu["S"])
+        bc = jf_bc()
+        for f, fb in enumerate(case.bc):
+            b = bc.face[f]
+            b.type = int(fb.type)
+            b.T_wall = float(fb.T_wall)
+            for d in range(3):
+                b.u_wall[d] = float(fb.u_wall[d])
+            if fb.dirichlet is not None:
+                t = np.ascontiguousarray(np.asarray(fb.dirichlet, dtype=np.float64))
+                self._keep.append(t)
+                b.dirichlet = _dp(t)
+            if fb.dist is not None:
+                b.dist = jf_disturbance(1, fb.dist["A"], fb.dist["kappa"], fb.dist["t1_lo"], fb.dist["t1_hi"])
+        ga = np.asarray(case.body_accel, dtype=np.float64)
+        self._keep.append(ga)
+        self.stream = stream
+        sptr = C.c_void_p(stream.cuda_stream) if stream is not None else C.c_void_p(
+            torch.cuda.current_stream(self.device).cuda_stream)
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            st = L.jf_create(C.byref(h), C.byref(g), dt, case.gamma, case.R_gas, case.Pr, C.byref(mu),
+                             C.byref(bc), _dp(ga), C.c_void_p(ws_ptr), nbytes, sptr)
+        if st != JF_OK:
+            raise JFError(st, "jf_create")
+        self.h = h
+        nx, ny, nz = case.n
+        self.shape = (5, nz + 6, ny + 6, nx + 6)
+        assert L.jf_state_elems(h) == int(np.prod(self.shape))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().jf_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != JF_OK:
+            raise JFError(st, lib().jf_last_error(self.h).decode())
+
+    def _ptr(self, t):
+        assert t.is_cuda and t.dtype == self.tdtype and t.is_contiguous() and tuple(t.shape) == self.shape
+        return C.c_void_p(t.data_ptr())
+
+    def state(self, U0=None):
+        """Device copy of a host state array (case.U0 by default)."""
+        U = np.asarray(self.case.U0 if U0 is None else U0)
+        return self.torch.as_tensor(U, dtype=self.tdtype).contiguous().to(self.device)
+
+    def jf_fill_halo(self, U):
+        self._check(lib().jf_fill_halo(self.h, self._ptr(U)))
+        return U
+
+    def jf_rhs(self, U, R=None):
+        if R is None:
+            R = self.torch.zeros_like(U)
+        self._check(lib().jf_rhs(self.h, self._ptr(U), self._ptr(R)))
+        return R
+
+    def jf_rk3_step(self, U, dt):
+        self._check(lib().jf_rk3_step(self.h, self._ptr(U), float(dt)))
+        return U
+
+    def jf_cfl_dt(self, U, cfl):
+        dt = C.c_double()
+        st = lib().jf_cfl_dt(self.h, self._ptr(U), float(cfl), C.byref(dt))
+        return st, dt.value
+
+    def jf_diag_timing(self, enable):
+        self._check(lib().jf_diag_timing(self.h, int(bool(enable))))
+
+    def jf_diag_kernel_times(self):
+        """{kernel class name: (total ms, launches)} since the previous call (synchronises)."""
+        ms = (C.c_double * 6)()
+        n = (C.c_ulonglong * 6)()
+        self._check(lib().jf_diag_kernel_times(self.h, ms, n))
+        return {lib().jf_diag_kernel_name(k).decode(): (ms[k], int(n[k])) for k in range(6)}
+
+    def jf_launch_count(self):
+        return int(lib().jf_launch_count(self.h))
+
+
+def run_case(case, dtype="f64", n_steps=None, device="cuda:0", solver=None):
+    """Advance a case on the GPU the way the drivers do (mirror of the oracle-side driver in
+    tests): fixed dt x n_steps, or CFL steps clipped to t_end.  Returns (U tensor, list of dt)."""
+    s = solver or Solver(case, dtype, device)
+    U = s.state()
+    dts, t, step = [], 0.0, 0
+    n = n_steps if n_steps is not None else case.n_steps
+    while True:
+        if n is not None and step >= n:
+            break
+        if case.t_end is not None and t >= case.t_end * (1 - 1e-14):
+            break
+        if case.dt is not None:
+            dt = case.dt
+        else:
+            st, dt = s.jf_cfl_dt(U, case.cfl)
+            if st != JF_OK:
+                raise JFError(st, f"jf_cfl_dt at step {step}")
+            if case.t_end is not None:
+                dt = min(dt, case.t_end - t)
+        s.jf_rk3_step(U, dt)
+        t += dt
+        dts.append(dt)
+        step += 1
+    return U, dts

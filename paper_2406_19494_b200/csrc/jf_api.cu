@@ -1,0 +1,471 @@
+// jf_api.cu — C ABI of libjf (include/jf.h): argument validation, metric / BC tables, workspace
+// carving, kernel launches.  Host logic only; every step of the path runs in jf_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+#include <cuda_runtime.h>
+#include "../../include/jf.h"
+#include "jf_kernels.cuh"
+
+namespace {
+
+using jf::NH;
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Grid geometry (reading O2): widths, centres, halo geometry, index-space metrics.
+struct Metrics {
+  std::vector<double> dl[3], xc[3], Xc[3], Xf[3];
+};
+
+void build_metrics(const int n[3], const double* const xf[3], const bool periodic[3], Metrics& M) {
+  for (int a = 0; a < 3; ++a) {
+    const int N = n[a], P = N + 2 * NH;
+    std::vector<double>&d = M.dl[a], &x = M.xc[a];
+    d.assign(P, 0.0); x.assign(P, 0.0); M.Xc[a].assign(P, 1.0); M.Xf[a].assign(P, 1.0);
+    for (int i = 0; i < N; ++i) { d[i + NH] = xf[a][i + 1] - xf[a][i]; x[i + NH] = 0.5 * (xf[a][i] + xf[a][i + 1]); }
+    for (int m = 1; m <= NH; ++m) {
+      d[NH - m] = periodic[a] ? d[NH + N - m] : d[NH + m - 1];
+      d[NH + N - 1 + m] = periodic[a] ? d[NH + m - 1] : d[NH + N - m];
+    }
+    double e = xf[a][0];
+    for (int m = 1; m <= NH; ++m) { x[NH - m] = e - 0.5 * d[NH - m]; e -= d[NH - m]; }
+    e = xf[a][N];
+    for (int m = 1; m <= NH; ++m) { x[NH + N - 1 + m] = e + 0.5 * d[NH + N - 1 + m]; e += d[NH + N - 1 + m]; }
+    for (int p = NH; p < NH + N; ++p) M.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
+    for (int p = NH - 1; p < NH + N; ++p) M.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
+  }
+}
+
+struct Layout {  // byte offsets into the workspace
+  size_t tab_T[3][4];   // inv_dl, dl, i12Xc, i24Xf per axis (dtype)
+  size_t tab_xc[3];     // double
+  size_t dirichlet[6];  // double
+  size_t cfl;           // 4 x u64
+  size_t R, A, B, G;    // fields (dtype)
+  size_t total;
+};
+
+Layout make_layout(const int n[3], size_t esz) {
+  Layout L;
+  size_t off = 0;
+  for (int a = 0; a < 3; ++a) {
+    for (int t = 0; t < 4; ++t) { L.tab_T[a][t] = off; off = align_up(off + (size_t)(n[a] + 6) * esz); }
+    L.tab_xc[a] = off; off = align_up(off + (size_t)(n[a] + 6) * sizeof(double));
+  }
+  for (int f = 0; f < 6; ++f) {
+    int a = f / 2, t1 = (a == 0) ? 1 : 0, t2 = (a == 2) ? 1 : 2;
+    L.dirichlet[f] = off; off = align_up(off + (size_t)5 * n[t1] * n[t2] * sizeof(double));
+  }
+  L.cfl = off; off = align_up(off + 4 * sizeof(unsigned long long));
+  size_t vol = (size_t)(n[0] + 6) * (n[1] + 6) * (n[2] + 6);
+  L.R = off; off = align_up(off + 5 * vol * esz);
+  L.A = off; off = align_up(off + 5 * vol * esz);
+  L.B = off; off = align_up(off + 5 * vol * esz);
+  L.G = off; off = align_up(off + 9 * vol * esz);
+  L.total = off;
+  return L;
+}
+
+bool grid_ok(const jf_grid* g) {
+  if (!g || g->nx < 4 || g->ny < 4 || g->nz < 4 || !g->xf || !g->yf || !g->zf) return false;
+  const double* xf[3] = {g->xf, g->yf, g->zf};
+  const int n[3] = {g->nx, g->ny, g->nz};
+  for (int a = 0; a < 3; ++a)
+    for (int i = 0; i < n[a]; ++i)
+      if (!(xf[a][i + 1] > xf[a][i])) return false;
+  return true;
+}
+
+template <class T>
+struct Impl {
+  jf::Params<T> P;
+  jf::FaceBC<T> bc[6];
+  T *R, *A, *B, *G;
+  unsigned long long* cfl_out;
+};
+
+}  // namespace
+
+struct jf_solver {
+  jf_dtype dtype;
+  Impl<double> d;
+  Impl<float> f;
+  cudaStream_t stream;
+  bool viscous;
+  double Pr;
+  std::string err;
+  unsigned long long launches;
+  int seg_len[3];
+  // optional per-kernel timing (jf_diag_timing): CUDA events around every launch
+  bool timing = false;
+  struct Ev { cudaEvent_t a, b; int cls; };
+  std::vector<Ev> ev_used, ev_free;
+};
+
+enum { K_HALO = 0, K_GRAD = 1, K_SWEEP_X = 2, K_SWEEP_Y = 3, K_SWEEP_Z = 4, K_CFL = 5, K_COUNT = 6 };
+
+namespace {
+
+jf_status fail(jf_solver* s, jf_status st, const char* what, cudaError_t ce = cudaSuccess) {
+  if (s) {
+    s->err = what;
+    if (ce != cudaSuccess) { s->err += ": "; s->err += cudaGetErrorString(ce); }
+  }
+  return st;
+}
+
+// RAII: records an event pair around one kernel launch when timing is on.
+struct Timed {
+  jf_solver* s; jf_solver::Ev e; bool on;
+  Timed(jf_solver* s_, int cls) : s(s_), on(s_->timing) {
+    if (!on) return;
+    if (!s->ev_free.empty()) { e = s->ev_free.back(); s->ev_free.pop_back(); }
+    else { cudaEventCreate(&e.a); cudaEventCreate(&e.b); }
+    e.cls = cls;
+    cudaEventRecord(e.a, s->stream);
+  }
+  ~Timed() {
+    if (!on) return;
+    cudaEventRecord(e.b, s->stream);
+    s->ev_used.push_back(e);
+  }
+};
+
+#define JF_CUDA(s, call)                                                  \
+  do {                                                                    \
+    cudaError_t ce_ = (call);                                             \
+    if (ce_ != cudaSuccess) return fail((s), JF_ECUDA, #call, ce_);       \
+  } while (0)
+
+template <class T>
+jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double R_gas, double Pr,
+                const jf_mu_law* mu, const jf_bc* bc, const double* ga, char* ws) {
+  const int n[3] = {g->nx, g->ny, g->nz};
+  const double* xf[3] = {g->xf, g->yf, g->zf};
+  bool per[3];
+  for (int a = 0; a < 3; ++a) per[a] = bc->face[2 * a].type == JF_BC_PERIODIC;
+  Metrics M;
+  build_metrics(n, xf, per, M);
+  Layout L = make_layout(n, sizeof(T));
+  jf::Params<T>& P = I.P;
+  for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
+  P.sy = P.P[0]; P.sz = (long long)P.P[0] * P.P[1]; P.vol = P.sz * P.P[2];
+  jf::Gas<T>& G = P.gas;
+  G.gamma = T(gamma); G.gm1 = T(gamma - 1.0); G.inv_gm1 = T(1.0 / (gamma - 1.0));
+  G.Rgas = T(R_gas); G.inv_Rgas = T(1.0 / R_gas);
+  G.mu_ref = T(mu->mu_ref); G.inv_T_ref = T(1.0 / mu->T_ref); G.S = T(mu->S); G.TrefS = T(mu->T_ref + mu->S);
+  G.lam_fac = T(gamma * R_gas / (gamma - 1.0) / Pr); G.Pr = T(Pr);
+  G.sutherland = mu->sutherland != 0; G.viscous = mu->mu_ref > 0.0;
+  for (int a = 0; a < 3; ++a) G.g[a] = T(ga ? ga[a] : 0.0);
+  for (int a = 0; a < 3; ++a) {
+    const int Pn = n[a] + 6;
+    std::vector<T> t[4];
+    for (int k = 0; k < 4; ++k) t[k].resize(Pn);
+    for (int p = 0; p < Pn; ++p) {
+      t[0][p] = T(1.0 / M.dl[a][p]); t[1][p] = T(M.dl[a][p]);
+      t[2][p] = T(1.0 / (12.0 * M.Xc[a][p])); t[3][p] = T(1.0 / (24.0 * M.Xf[a][p]));
+    }
+    for (int k = 0; k < 4; ++k)
+      JF_CUDA(s, cudaMemcpy(ws + L.tab_T[a][k], t[k].data(), Pn * sizeof(T), cudaMemcpyHostToDevice));
+    JF_CUDA(s, cudaMemcpy(ws + L.tab_xc[a], M.xc[a].data(), Pn * sizeof(double), cudaMemcpyHostToDevice));
+    P.inv_dl[a] = (const T*)(ws + L.tab_T[a][0]); P.dl[a] = (const T*)(ws + L.tab_T[a][1]);
+    P.i12Xc[a] = (const T*)(ws + L.tab_T[a][2]); P.i24Xf[a] = (const T*)(ws + L.tab_T[a][3]);
+    P.xc[a] = (const double*)(ws + L.tab_xc[a]);
+  }
+  for (int f = 0; f < 6; ++f) {
+    const jf_bc_face& b = bc->face[f];
+    jf::FaceBC<T>& o = I.bc[f];
+    o.type = (int)b.type; o.T_wall = T(b.T_wall);
+    for (int d = 0; d < 3; ++d) o.uw[d] = T(b.u_wall[d]);
+    const bool wall = b.type == JF_BC_WALL_ISOTHERMAL || b.type == JF_BC_WALL_ADIABATIC;
+    o.dist_on = wall && b.dist.enabled;
+    o.A = b.dist.A; o.kappa = b.dist.kappa; o.lo = b.dist.t1_lo; o.hi = b.dist.t1_hi;
+    o.dirichlet = nullptr;
+    if (b.type == JF_BC_DIRICHLET) {
+      int a = f / 2, t1 = (a == 0) ? 1 : 0, t2 = (a == 2) ? 1 : 2;
+      JF_CUDA(s, cudaMemcpy(ws + L.dirichlet[f], b.dirichlet, (size_t)5 * n[t1] * n[t2] * sizeof(double),
+                            cudaMemcpyHostToDevice));
+      o.dirichlet = (const double*)(ws + L.dirichlet[f]);
+    }
+  }
+  I.R = (T*)(ws + L.R); I.A = (T*)(ws + L.A); I.B = (T*)(ws + L.B); I.G = (T*)(ws + L.G);
+  I.cfl_out = (unsigned long long*)(ws + L.cfl);
+  return JF_OK;
+}
+
+int pick_segment(long long columns, int N) {
+  // enough independent columns x segments to fill 148 SMs several times over
+  int L = 32;
+  while (L > 8 && columns * ((N + L - 1) / L) < 148LL * 2048 * 2) L /= 2;
+  return L < N ? L : N;
+}
+
+template <class T>
+jf_status launch_halo(jf_solver* s, Impl<T>& I, T* U) {
+  const jf::Params<T>& P = I.P;
+  {
+    Timed t(s, K_HALO);
+    long long tot = (long long)P.n[1] * P.n[2] * 6;
+    jf::halo_kernel<T, 0><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[0], I.bc[1], U);
+  }
+  {
+    Timed t(s, K_HALO);
+    long long tot = (long long)P.P[0] * P.n[2] * 6;
+    jf::halo_kernel<T, 1><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[2], I.bc[3], U);
+  }
+  {
+    Timed t(s, K_HALO);
+    long long tot = (long long)P.P[0] * P.P[1] * 6;
+    jf::halo_kernel<T, 2><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[4], I.bc[5], U);
+  }
+  s->launches += 3;
+  JF_CUDA(s, cudaPeekAtLastError());
+  return JF_OK;
+}
+
+// R_NSE of Eq. 6.  rk == nullptr: R <- R_NSE(U).  Otherwise the z sweep applies the RK stage.
+template <class T, bool VISC>
+jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
+  const jf::Params<T>& P = I.P;
+  const T* G = VISC ? I.G : nullptr;
+  if (VISC) {
+    Timed t(s, K_GRAD);
+    dim3 grid((P.P[0] + 255) / 256, P.P[1], P.P[2]);
+    jf::gradient_kernel<T><<<grid, 256, 0, s->stream>>>(P, U, I.G);
+    s->launches += 1;
+  }
+  {
+    Timed t(s, K_SWEEP_X);
+    const int rows = P.n[1] * P.n[2];
+    const size_t sh = (size_t)jf::XS_WARPS * 6 * 64 * sizeof(T);
+    jf::sweep_x_kernel<T, VISC><<<(rows + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
+  }
+  const size_t sh = (size_t)6 * 6 * jf::YZ_TX * jf::YZ_TY * sizeof(T);
+  const dim3 blk(jf::YZ_TX, jf::YZ_TY);
+  jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0)};
+  {
+    Timed t(s, K_SWEEP_Y);
+    const int L = s->seg_len[1];
+    dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, (P.n[2] + jf::YZ_TY - 1) / jf::YZ_TY, (P.n[1] + L - 1) / L);
+    jf::sweep_yz_kernel<T, 1, VISC, 0><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
+  }
+  {
+    Timed t(s, K_SWEEP_Z);
+    const int L = s->seg_len[2];
+    dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, (P.n[1] + jf::YZ_TY - 1) / jf::YZ_TY, (P.n[2] + L - 1) / L);
+    if (rk) jf::sweep_yz_kernel<T, 2, VISC, 2><<<grid, blk, sh, s->stream>>>(P, U, G, R, *rk, L);
+    else jf::sweep_yz_kernel<T, 2, VISC, 1><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
+  }
+  s->launches += 3;
+  JF_CUDA(s, cudaPeekAtLastError());
+  return JF_OK;
+}
+
+template <class T>
+jf_status launch_rhs(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
+  return s->viscous ? launch_rhs_t<T, true>(s, I, U, R, rk) : launch_rhs_t<T, false>(s, I, U, R, rk);
+}
+
+template <class T>
+jf_status rk3(jf_solver* s, Impl<T>& I, T* U, double dt) {
+  jf_status st;
+  // stage 1: A = U + dt L(U)
+  if ((st = launch_halo<T>(s, I, U))) return st;
+  jf::RKArgs<T> r1{U, I.A, T(0), T(1), T(dt)};
+  if ((st = launch_rhs<T>(s, I, U, I.R, &r1))) return st;
+  // stage 2: B = 3/4 U + 1/4 (A + dt L(A))
+  if ((st = launch_halo<T>(s, I, I.A))) return st;
+  jf::RKArgs<T> r2{U, I.B, T(0.75), T(0.25), T(dt)};
+  if ((st = launch_rhs<T>(s, I, I.A, I.R, &r2))) return st;
+  // stage 3: U = 1/3 U + 2/3 (B + dt L(B))   (pointwise in place: each thread reads U^n then writes)
+  if ((st = launch_halo<T>(s, I, I.B))) return st;
+  jf::RKArgs<T> r3{U, U, T(1.0 / 3.0), T(2.0 / 3.0), T(dt)};
+  return launch_rhs<T>(s, I, I.B, I.R, &r3);
+}
+
+template <class T>
+jf_status cfl(jf_solver* s, Impl<T>& I, const T* U, double cflnum, double* dt_host) {
+  JF_CUDA(s, cudaMemsetAsync(I.cfl_out, 0xFF, 3 * sizeof(unsigned long long), s->stream));
+  JF_CUDA(s, cudaMemsetAsync(I.cfl_out + 3, 0, sizeof(unsigned long long), s->stream));
+  long long ncell = (long long)I.P.n[0] * I.P.n[1] * I.P.n[2];
+  int blocks = (int)std::min<long long>((ncell + 255) / 256, 148LL * 8);
+  {
+    Timed t(s, K_CFL);
+    jf::cfl_kernel<T><<<blocks, 256, 0, s->stream>>>(I.P, U, I.cfl_out);
+  }
+  s->launches += 1;
+  JF_CUDA(s, cudaPeekAtLastError());
+  unsigned long long h[4];
+  JF_CUDA(s, cudaMemcpyAsync(h, I.cfl_out, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  if (h[3]) { *dt_host = std::nan(""); return fail(s, JF_ENOTFINITE, "jf_cfl_dt: non-finite state or rho <= 0 or p <= 0"); }
+  double v[3];
+  std::memcpy(v, h, sizeof(v));
+  double dt = v[0];
+  if (s->viscous) dt = std::fmin(dt, std::fmin((3.0 / 14.0) * v[1], (1.0 / 10.0) * v[2]));
+  *dt_host = cflnum * dt;
+  return JF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t jf_workspace_bytes(const jf_grid* g, jf_dtype dtype) {
+  if (!grid_ok(g) || (dtype != JF_F64 && dtype != JF_F32)) return 0;
+  const int n[3] = {g->nx, g->ny, g->nz};
+  return make_layout(n, dtype == JF_F64 ? sizeof(double) : sizeof(float)).total;
+}
+
+jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double gamma, double R_gas, double Pr,
+                    const jf_mu_law* mu, const jf_bc* bc, const double body_accel[3], void* workspace_dev,
+                    size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return JF_EINVAL;
+  *out = nullptr;
+  if (!grid_ok(g) || !mu || !bc) return JF_EINVAL;
+  if (dtype != JF_F64 && dtype != JF_F32) return JF_EINVAL;
+  if (!(gamma > 1.0) || !(R_gas > 0.0) || !(Pr > 0.0) || !(mu->mu_ref >= 0.0)) return JF_EINVAL;
+  if (mu->sutherland && !(mu->T_ref > 0.0)) return JF_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if ((bc->face[2 * a].type == JF_BC_PERIODIC) != (bc->face[2 * a + 1].type == JF_BC_PERIODIC)) return JF_EINVAL;
+  for (int f = 0; f < 6; ++f) {
+    const jf_bc_face& b = bc->face[f];
+    if ((int)b.type < 0 || (int)b.type > 4) return JF_EINVAL;
+    if (b.type == JF_BC_DIRICHLET && !b.dirichlet) return JF_EINVAL;
+    if (b.type == JF_BC_WALL_ISOTHERMAL && !(b.T_wall > 0.0)) return JF_EINVAL;
+  }
+  if (!workspace_dev) return JF_EWORKSPACE;
+  if (((uintptr_t)workspace_dev) % 256 != 0) return JF_EALIGN;
+  if (workspace_bytes < jf_workspace_bytes(g, dtype)) return JF_EWORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return JF_ECUDA;  // no CPU fallback
+  jf_solver* s = new (std::nothrow) jf_solver();
+  if (!s) return JF_EINVAL;
+  s->dtype = dtype;
+  s->stream = (cudaStream_t)cuda_stream;
+  s->viscous = mu->mu_ref > 0.0;
+  s->Pr = Pr;
+  s->launches = 0;
+  jf_status st = dtype == JF_F64
+                     ? setup<double>(s, s->d, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev)
+                     : setup<float>(s, s->f, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev);
+  if (st != JF_OK) { delete s; return st; }
+  const int n[3] = {g->nx, g->ny, g->nz};
+  s->seg_len[0] = 0;
+  s->seg_len[1] = pick_segment((long long)n[0] * n[2], n[1]);
+  s->seg_len[2] = pick_segment((long long)n[0] * n[1], n[2]);
+  *out = s;
+  return JF_OK;
+}
+
+jf_status jf_destroy(jf_solver* s) {
+  if (s) {
+    for (auto& e : s->ev_used) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (auto& e : s->ev_free) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  }
+  delete s;
+  return JF_OK;
+}
+
+jf_status jf_diag_timing(jf_solver* s, int enable) {
+  if (!s) return JF_EINVAL;
+  s->timing = enable != 0;
+  return JF_OK;
+}
+
+jf_status jf_diag_kernel_times(jf_solver* s, double ms[6], unsigned long long launches[6]) {
+  if (!s || !ms || !launches) return JF_EINVAL;
+  for (int k = 0; k < K_COUNT; ++k) { ms[k] = 0.0; launches[k] = 0; }
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  for (auto& e : s->ev_used) {
+    float t = 0.f;
+    JF_CUDA(s, cudaEventElapsedTime(&t, e.a, e.b));
+    ms[e.cls] += t; launches[e.cls] += 1;
+    s->ev_free.push_back(e);
+  }
+  s->ev_used.clear();
+  return JF_OK;
+}
+
+const char* jf_diag_kernel_name(int k) {
+  static const char* names[K_COUNT] = {"halo_kernel", "gradient_kernel", "sweep_x_kernel", "sweep_yz_kernel<y>",
+                                       "sweep_yz_kernel<z>+rk", "cfl_kernel"};
+  return (k >= 0 && k < K_COUNT) ? names[k] : "";
+}
+
+size_t jf_state_elems(const jf_solver* s) {
+  if (!s) return 0;
+  return s->dtype == JF_F64 ? (size_t)5 * s->d.P.vol : (size_t)5 * s->f.P.vol;
+}
+
+static bool aligned16(const void* p) { return ((uintptr_t)p) % 16 == 0; }
+
+jf_status jf_fill_halo(jf_solver* s, void* U) {
+  if (!s) return JF_EINVAL;
+  if (!U) return fail(s, JF_EINVAL, "jf_fill_halo: null pointer");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_fill_halo: U not 16-byte aligned");
+  return s->dtype == JF_F64 ? launch_halo<double>(s, s->d, (double*)U) : launch_halo<float>(s, s->f, (float*)U);
+}
+
+jf_status jf_rhs(jf_solver* s, const void* U, void* R) {
+  if (!s) return JF_EINVAL;
+  if (!U || !R || U == R) return fail(s, JF_EINVAL, "jf_rhs: null or aliased pointers");
+  if (!aligned16(U) || !aligned16(R)) return fail(s, JF_EALIGN, "jf_rhs: pointer not 16-byte aligned");
+  return s->dtype == JF_F64 ? launch_rhs<double>(s, s->d, (const double*)U, (double*)R, nullptr)
+                            : launch_rhs<float>(s, s->f, (const float*)U, (float*)R, nullptr);
+}
+
+jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
+  if (!s) return JF_EINVAL;
+  if (!U || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_step: null pointer or NaN dt");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_step: U not 16-byte aligned");
+  return s->dtype == JF_F64 ? rk3<double>(s, s->d, (double*)U, dt) : rk3<float>(s, s->f, (float*)U, dt);
+}
+
+jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host) {
+  if (!s) return JF_EINVAL;
+  if (!U || !dt_host) return fail(s, JF_EINVAL, "jf_cfl_dt: null pointer");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_cfl_dt: U not 16-byte aligned");
+  return s->dtype == JF_F64 ? cfl<double>(s, s->d, (const double*)U, cflnum, dt_host)
+                            : cfl<float>(s, s->f, (const float*)U, cflnum, dt_host);
+}
+
+const char* jf_last_error(const jf_solver* s) { return s ? s->err.c_str() : ""; }
+
+unsigned long long jf_launch_count(const jf_solver* s) { return s ? s->launches : 0ULL; }
+
+jf_status jf_diag_alu_peak(jf_dtype dtype, int iters, double* flops_host, double* ms_host) {
+  if (!flops_host || iters <= 0 || (dtype != JF_F64 && dtype != JF_F32)) return JF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return JF_ECUDA;
+  void* buf = nullptr;
+  if (cudaMalloc(&buf, 256) != cudaSuccess) return JF_ECUDA;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 148 * 8, threads = 256;
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    if (dtype == JF_F64) jf::alu_peak_kernel<double><<<blocks, threads>>>((double*)buf, iters, 1.0);
+    else jf::alu_peak_kernel<float><<<blocks, threads>>>((float*)buf, iters, 1.0f);
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(buf); return JF_ECUDA; }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(buf);
+  double fl = 2.0 * 64.0 * (double)iters * (double)blocks * threads;
+  *flops_host = fl / (best * 1e-3);
+  if (ms_host) *ms_host = best;
+  return cudaGetLastError() == cudaSuccess ? JF_OK : JF_ECUDA;
+}
+
+const char* jf_version(void) { return "libjf 0.1 (sm_100a; WENO5-JS + HLLC + 4th-order viscous + SSP-RK3)"; }
+
+}  // extern "C"

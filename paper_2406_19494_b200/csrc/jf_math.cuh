@@ -1,0 +1,165 @@
+// jf_math.cuh — per-face device arithmetic of the hot path (sm_100a).
+//
+// Written for the plain FP64/FP32 ALUs (nothing here is a dense contraction, so no tensor
+// cores): the formulas of DESIGN.md "Readings" (WENO5-JS, HLLC with Roe-average wave speeds,
+// 4th-order central dissipative flux, Sutherland) restructured to cut divisions — the FP64
+// pipe pays ~10 issue slots per division:
+//   * WENO5: the three non-linear weights are formed as products n_k = d_k e_l e_m with
+//     e_k = (beta_k + eps)^2, so one reconstruction costs ONE division instead of four;
+//   * HLLC: only the star state on the side selected by sign(S*) is evaluated (the other is
+//     multiplied by an exact zero in the closed form), reciprocals are shared.
+// Results agree with the closed forms to a few ulp, not bit-wise (tolerance: DESIGN.md).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace jf {
+
+template <class T> struct Num;
+template <> struct Num<double> {
+  static __device__ __forceinline__ double sqrt_(double a) { return sqrt(a); }
+  static __device__ __forceinline__ double rcp(double a) { return 1.0 / a; }
+  static __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
+  static __device__ __forceinline__ double min_(double a, double b) { return fmin(a, b); }
+  static __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
+  static __device__ __forceinline__ double abs_(double a) { return fabs(a); }
+};
+template <> struct Num<float> {
+  static __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
+  static __device__ __forceinline__ float rcp(float a) { return 1.0f / a; }
+  static __device__ __forceinline__ float rsqrt_(float a) { return 1.0f / sqrtf(a); }
+  static __device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
+  static __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
+  static __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
+};
+
+// gas / transport constants handed to every kernel
+template <class T>
+struct Gas {
+  T gamma, gm1, inv_gm1, Rgas, inv_Rgas;
+  T mu_ref, inv_T_ref, S, TrefS;  // TrefS = T_ref + S
+  T lam_fac;                      // lambda = mu * lam_fac, lam_fac = cp/Pr = gamma R/((gamma-1) Pr)
+  T Pr;
+  int sutherland, viscous;
+  T g[3];
+};
+
+// Eq. 2: conservative -> (rho,u,v,w,p,T)
+template <class T>
+__device__ __forceinline__ void cons_to_prim(const Gas<T>& gas, T r, T mx, T my, T mz, T E, T W[6]) {
+  T ri = Num<T>::rcp(r);
+  T u = mx * ri, v = my * ri, w = mz * ri;
+  T p = gas.gm1 * (E - T(0.5) * (mx * u + my * v + mz * w));
+  W[0] = r; W[1] = u; W[2] = v; W[3] = w; W[4] = p;
+  W[5] = p * ri * gas.inv_Rgas;
+}
+
+// Sutherland: mu = mu_ref r sqrt(r) (T_ref+S)/(T+S), r = T/T_ref
+template <class T>
+__device__ __forceinline__ T viscosity(const Gas<T>& gas, T Tf) {
+  if (!gas.sutherland) return gas.mu_ref;
+  T r = Tf * gas.inv_T_ref;
+  return gas.mu_ref * (r * Num<T>::sqrt_(r)) * gas.TrefS * Num<T>::rcp(Tf + gas.S);
+}
+
+// WENO5-JS value at the face between v2 and v3; one division.
+template <class T>
+__device__ __forceinline__ T weno5(T v0, T v1, T v2, T v3, T v4) {
+  const T eps = T(1e-6), c1312 = T(13.0 / 12.0);
+  T a0 = v0 - T(2) * v1 + v2, b0 = v0 - T(4) * v1 + T(3) * v2;
+  T a1 = v1 - T(2) * v2 + v3, b1 = v1 - v3;
+  T a2 = v2 - T(2) * v3 + v4, b2 = T(3) * v2 - T(4) * v3 + v4;
+  T e0 = c1312 * (a0 * a0) + T(0.25) * (b0 * b0) + eps;
+  T e1 = c1312 * (a1 * a1) + T(0.25) * (b1 * b1) + eps;
+  T e2 = c1312 * (a2 * a2) + T(0.25) * (b2 * b2) + eps;
+  e0 *= e0; e1 *= e1; e2 *= e2;
+  T n0 = T(0.1) * (e1 * e2), n1 = T(0.6) * (e0 * e2), n2 = T(0.3) * (e0 * e1);
+  T q0 = T(2) * v0 - T(7) * v1 + T(11) * v2;
+  T q1 = T(5) * v2 - v1 + T(2) * v3;
+  T q2 = T(2) * v2 + T(5) * v3 - v4;
+  T num = n0 * q0 + n1 * q1 + n2 * q2;
+  T den = T(6) * (n0 + n1 + n2);
+  return num / den;
+}
+
+// HLLC flux in the rotated frame: states (rho, un, ut1, ut2, p) -> F = [mass, n, t1, t2, energy]
+template <class T>
+__device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const T R[5], T F[5]) {
+  using N = Num<T>;
+  T tL = N::rsqrt_(L[0]), tR = N::rsqrt_(R[0]);        // 1/sqrt(rho)
+  T sL = L[0] * tL, sR = R[0] * tR;                      // sqrt(rho)
+  T riL = tL * tL, riR = tR * tR;                        // 1/rho
+  T cL = N::sqrt_(gas.gamma * L[4]) * tL, cR = N::sqrt_(gas.gamma * R[4]) * tR;
+  T qL = L[1] * L[1] + L[2] * L[2] + L[3] * L[3], qR = R[1] * R[1] + R[2] * R[2] + R[3] * R[3];
+  T EL = L[4] * gas.inv_gm1 + T(0.5) * L[0] * qL, ER = R[4] * gas.inv_gm1 + T(0.5) * R[0] * qR;
+  T HL = (EL + L[4]) * riL, HR = (ER + R[4]) * riR;
+  T rs = N::rcp(sL + sR);
+  T wL = sL * rs, wR = sR * rs;
+  T un = wL * L[1] + wR * R[1], u1 = wL * L[2] + wR * R[2], u2 = wL * L[3] + wR * R[3];
+  T Ht = wL * HL + wR * HR;
+  T ct = N::sqrt_(gas.gm1 * (Ht - T(0.5) * (un * un + u1 * u1 + u2 * u2)));
+  T SL = N::min_(L[1] - cL, un - ct), SR = N::max_(R[1] + cR, un + ct);
+  T mL = L[0] * (SL - L[1]), mR = R[0] * (SR - R[1]);
+  T Ss = (R[4] - L[4] + L[1] * mL - R[1] * mR) / (mL - mR);
+  // side selected by sign(S*)  (S* == 0: both star fluxes are mathematically equal)
+  bool left = Ss >= T(0);
+  T rho = left ? L[0] : R[0], vn = left ? L[1] : R[1], v1 = left ? L[2] : R[2], v2 = left ? L[3] : R[3];
+  T p = left ? L[4] : R[4], E = left ? EL : ER, SK = left ? SL : SR, m = left ? mL : mR;
+  T ri = left ? riL : riR;
+  T Sc = left ? N::min_(SL, T(0)) : N::max_(SR, T(0));  // min(S_L,0) / max(S_R,0)
+  T mn = rho * vn;
+  T F0 = mn, F1 = mn * vn + p, F2 = mn * v1, F3 = mn * v2, F4 = vn * (E + p);
+  T dinv = N::rcp(SK - Ss);
+  T fac = m * dinv;
+  T dS = Ss - vn;
+  T Es = fac * (E * ri + dS * Ss) + dS * p * dinv;       // fac*(E/rho + dS*(S* + p/m))
+  F[0] = F0 + Sc * (fac - rho);
+  F[1] = F1 + Sc * (fac * Ss - mn);
+  F[2] = F2 + Sc * (fac * v1 - rho * v1);
+  F[3] = F3 + Sc * (fac * v2 - rho * v2);
+  F[4] = F4 + Sc * (Es - E);
+}
+
+// Total face flux (convective - dissipative, Eq. 6) of the face between cells 0 and +1 along DIR.
+//   w(m, q): primitive q in {rho,u,v,w,p,T} of the cell at offset m in -2..3 along DIR
+//   g(m, c): transverse centre derivatives at offset m in -1..2:
+//            c = 0: d_t1 u_n, 1: d_t1 u_t1, 2: d_t2 u_n, 3: d_t2 u_t2
+//   i24Xf: 1/(24 X_xi^f) of this face.   (n,t1,t2) = (DIR, DIR+1, DIR+2) mod 3.
+template <class T, int DIR, bool VISC, class WAcc, class GAcc>
+__device__ __forceinline__ void face_flux(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T F[5]) {
+  constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  constexpr int qs[5] = {0, 1 + n, 1 + t1, 1 + t2, 4};
+  T L[5], R[5];
+#pragma unroll
+  for (int c = 0; c < 5; ++c) {
+    const int q = qs[c];
+    T s0 = w(-2, q), s1 = w(-1, q), s2 = w(0, q), s3 = w(1, q), s4 = w(2, q), s5 = w(3, q);
+    L[c] = weno5<T>(s0, s1, s2, s3, s4);
+    R[c] = weno5<T>(s5, s4, s3, s2, s1);
+  }
+  T Fr[5];
+  hllc_rot<T>(gas, L, R, Fr);
+  if (VISC) {
+    T dn[4], fv[4];  // normal derivative and face value of u_n, u_t1, u_t2, T
+    constexpr int qv[4] = {1 + n, 1 + t1, 1 + t2, 5};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      T m1 = w(-1, qv[c]), c0 = w(0, qv[c]), p1 = w(1, qv[c]), p2 = w(2, qv[c]);
+      dn[c] = (T(27) * (p1 - c0) - (p2 - m1)) * i24Xf;
+      fv[c] = (T(9) * (c0 + p1) - (m1 + p2)) * T(1.0 / 16.0);
+    }
+    T gt[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      gt[c] = (T(9) * (g(0, c) + g(1, c)) - (g(-1, c) + g(2, c))) * T(1.0 / 16.0);
+    T mu = viscosity<T>(gas, fv[3]);
+    T div = dn[0] + gt[1] + gt[3];
+    T tnn = mu * (T(2) * dn[0] - T(2.0 / 3.0) * div);
+    T tn1 = mu * (gt[0] + dn[1]);
+    T tn2 = mu * (gt[2] + dn[2]);
+    Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
+    Fr[4] -= fv[0] * tnn + fv[1] * tn1 + fv[2] * tn2 + mu * gas.lam_fac * dn[3];
+  }
+  F[0] = Fr[0]; F[1 + n] = Fr[1]; F[1 + t1] = Fr[2]; F[1 + t2] = Fr[3]; F[4] = Fr[4];
+}
+
+}  // namespace jf
