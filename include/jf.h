@@ -135,6 +135,16 @@ jf_status jf_diag_timing(jf_solver *s, int enable);
 jf_status jf_diag_kernel_times(jf_solver *s, double ms[6], unsigned long long launches[6]);
 const char *jf_diag_kernel_name(int k);
 
+/* Unit-level diagnostic of the per-face arithmetic the sweep kernels use (not on the hot path):
+ * total face flux F = F^c - F^d (Eq. 6) along dir for n_faces independent faces.  HOST arrays:
+ * W[n][6][6] primitives (rho,u,v,w,p,T) of the six cells i-2..i+3 around each face, Gt[n][4][4]
+ * transverse centre derivatives at cells i-1..i+2 (d_t1 u_n, d_t1 u_t1, d_t2 u_n, d_t2 u_t2;
+ * may be NULL = 0), Xf[n] face metric X_xi^f (NULL = 1), F[n][5] output.  Dissipative part only
+ * if mu->mu_ref > 0.  Allocates its own scratch; synchronises. */
+jf_status jf_diag_face_flux(jf_dtype dtype, int dir, double gamma, double R_gas, double Pr,
+                            const jf_mu_law *mu, int n_faces, const double *W, const double *Gt,
+                            const double *Xf, double *F);
+
 /* Library version / build info string (static storage). */
 const char *jf_version(void);
 

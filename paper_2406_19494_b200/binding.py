@@ -44,7 +44,7 @@ class jf_bc(C.Structure):
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
            "jf_rk3_step", "jf_cfl_dt", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
-           "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_version"]
+           "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_version"]
 
 _lib = None
 
@@ -92,6 +92,9 @@ def lib():
         L.jf_diag_kernel_times.argtypes = [C.c_void_p, c_double_p, C.POINTER(C.c_ulonglong)]
         L.jf_diag_kernel_name.restype = C.c_char_p
         L.jf_diag_kernel_name.argtypes = [C.c_int]
+        L.jf_diag_face_flux.restype = C.c_int
+        L.jf_diag_face_flux.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(jf_mu_law),
+                                        C.c_int, c_double_p, c_double_p, c_double_p, c_double_p]
         L.jf_version.restype = C.c_char_p
         L.jf_version.argtypes = []
         _lib = L
@@ -119,6 +122,22 @@ def jf_diag_alu_peak(dtype="f64", iters=4096):
     if st != JF_OK:
         raise JFError(st, "jf_diag_alu_peak")
     return fl.value, ms.value
+
+
+def jf_diag_face_flux(dtype, d, gamma, R_gas, Pr, mu, W, Gt=None, Xf=None):
+    """F[n,5] = total face flux of n faces from W[n,6,6], Gt[n,4,4], Xf[n] (host numpy arrays)."""
+    W = np.ascontiguousarray(W, dtype=np.float64)
+    n = W.shape[0]
+    assert W.shape == (n, 6, 6)
+    Gt = None if Gt is None else np.ascontiguousarray(Gt, dtype=np.float64)
+    Xf = None if Xf is None else np.ascontiguousarray(Xf, dtype=np.float64)
+    F = np.zeros((n, 5))
+    m = jf_mu_law(int(mu["sutherland"]), mu["mu_ref"], mu["T_ref"], mu["S"])
+    st = lib().jf_diag_face_flux(JF_F64 if dtype == "f64" else JF_F32, d, gamma, R_gas, Pr, C.byref(m), n, _dp(W),
+                                 None if Gt is None else _dp(Gt), None if Xf is None else _dp(Xf), _dp(F))
+    if st != JF_OK:
+        raise JFError(st, "jf_diag_face_flux")
+    return F
 
 
 class Solver:

@@ -142,6 +142,44 @@ struct Timed {
   } while (0)
 
 template <class T>
+void fill_gas(jf::Gas<T>& G, double gamma, double R_gas, double Pr, const jf_mu_law* mu, const double* ga) {
+  G.gamma = T(gamma); G.gm1 = T(gamma - 1.0); G.inv_gm1 = T(1.0 / (gamma - 1.0));
+  G.Rgas = T(R_gas); G.inv_Rgas = T(1.0 / R_gas);
+  G.mu_ref = T(mu->mu_ref); G.inv_T_ref = T(1.0 / mu->T_ref); G.S = T(mu->S); G.TrefS = T(mu->T_ref + mu->S);
+  G.lam_fac = T(gamma * R_gas / (gamma - 1.0) / Pr); G.Pr = T(Pr);
+  G.sutherland = mu->sutherland != 0; G.viscous = mu->mu_ref > 0.0;
+  for (int a = 0; a < 3; ++a) G.g[a] = T(ga ? ga[a] : 0.0);
+}
+
+template <class T>
+jf_status diag_face_flux(int dir, double gamma, double R_gas, double Pr, const jf_mu_law* mu, int nf,
+                         const double* W, const double* Gt, const double* Xf, double* F) {
+  jf::Gas<T> gas;
+  fill_gas<T>(gas, gamma, R_gas, Pr, mu, nullptr);
+  std::vector<T> hW((size_t)nf * 36), hG((size_t)nf * 16), hX(nf), hF((size_t)nf * 5);
+  for (size_t i = 0; i < hW.size(); ++i) hW[i] = T(W[i]);
+  for (size_t i = 0; i < hG.size(); ++i) hG[i] = T(Gt ? Gt[i] : 0.0);
+  for (int i = 0; i < nf; ++i) hX[i] = T(1.0 / (24.0 * (Xf ? Xf[i] : 1.0)));
+  T *dW = nullptr, *dG = nullptr, *dX = nullptr, *dF = nullptr;
+  bool ok = cudaMalloc(&dW, hW.size() * sizeof(T)) == cudaSuccess && cudaMalloc(&dG, hG.size() * sizeof(T)) == cudaSuccess &&
+            cudaMalloc(&dX, hX.size() * sizeof(T)) == cudaSuccess && cudaMalloc(&dF, hF.size() * sizeof(T)) == cudaSuccess;
+  if (ok) {
+    cudaMemcpy(dW, hW.data(), hW.size() * sizeof(T), cudaMemcpyHostToDevice);
+    cudaMemcpy(dG, hG.data(), hG.size() * sizeof(T), cudaMemcpyHostToDevice);
+    cudaMemcpy(dX, hX.data(), hX.size() * sizeof(T), cudaMemcpyHostToDevice);
+    const int blocks = (nf + 127) / 128;
+    if (dir == 0) jf::face_flux_kernel<T, 0><<<blocks, 128>>>(gas, dW, dG, dX, dF, nf);
+    else if (dir == 1) jf::face_flux_kernel<T, 1><<<blocks, 128>>>(gas, dW, dG, dX, dF, nf);
+    else jf::face_flux_kernel<T, 2><<<blocks, 128>>>(gas, dW, dG, dX, dF, nf);
+    ok = cudaMemcpy(hF.data(), dF, hF.size() * sizeof(T), cudaMemcpyDeviceToHost) == cudaSuccess;
+  }
+  cudaFree(dW); cudaFree(dG); cudaFree(dX); cudaFree(dF);
+  if (!ok) return JF_ECUDA;
+  for (size_t i = 0; i < hF.size(); ++i) F[i] = (double)hF[i];
+  return JF_OK;
+}
+
+template <class T>
 jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double R_gas, double Pr,
                 const jf_mu_law* mu, const jf_bc* bc, const double* ga, char* ws) {
   const int n[3] = {g->nx, g->ny, g->nz};
@@ -154,13 +192,7 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
   jf::Params<T>& P = I.P;
   for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
   P.sy = P.P[0]; P.sz = (long long)P.P[0] * P.P[1]; P.vol = P.sz * P.P[2];
-  jf::Gas<T>& G = P.gas;
-  G.gamma = T(gamma); G.gm1 = T(gamma - 1.0); G.inv_gm1 = T(1.0 / (gamma - 1.0));
-  G.Rgas = T(R_gas); G.inv_Rgas = T(1.0 / R_gas);
-  G.mu_ref = T(mu->mu_ref); G.inv_T_ref = T(1.0 / mu->T_ref); G.S = T(mu->S); G.TrefS = T(mu->T_ref + mu->S);
-  G.lam_fac = T(gamma * R_gas / (gamma - 1.0) / Pr); G.Pr = T(Pr);
-  G.sutherland = mu->sutherland != 0; G.viscous = mu->mu_ref > 0.0;
-  for (int a = 0; a < 3; ++a) G.g[a] = T(ga ? ga[a] : 0.0);
+  fill_gas<T>(P.gas, gamma, R_gas, Pr, mu, ga);
   for (int a = 0; a < 3; ++a) {
     const int Pn = n[a] + 6;
     std::vector<T> t[4];
@@ -464,6 +496,16 @@ jf_status jf_diag_alu_peak(jf_dtype dtype, int iters, double* flops_host, double
   *flops_host = fl / (best * 1e-3);
   if (ms_host) *ms_host = best;
   return cudaGetLastError() == cudaSuccess ? JF_OK : JF_ECUDA;
+}
+
+jf_status jf_diag_face_flux(jf_dtype dtype, int dir, double gamma, double R_gas, double Pr, const jf_mu_law* mu,
+                            int n_faces, const double* W, const double* Gt, const double* Xf, double* F) {
+  if (!mu || !W || !F || n_faces <= 0 || dir < 0 || dir > 2 || (dtype != JF_F64 && dtype != JF_F32)) return JF_EINVAL;
+  if (!(gamma > 1.0) || !(R_gas > 0.0) || !(Pr > 0.0)) return JF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return JF_ECUDA;
+  return dtype == JF_F64 ? diag_face_flux<double>(dir, gamma, R_gas, Pr, mu, n_faces, W, Gt, Xf, F)
+                         : diag_face_flux<float>(dir, gamma, R_gas, Pr, mu, n_faces, W, Gt, Xf, F);
 }
 
 const char* jf_version(void) { return "libjf 0.1 (sm_100a; WENO5-JS + HLLC + 4th-order viscous + SSP-RK3)"; }

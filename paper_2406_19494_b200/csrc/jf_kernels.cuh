@@ -371,6 +371,22 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
   }
 }
 
+// ------------------------------------------------------------------ diagnostics: one face flux per thread
+// W[f][6 cells][6 prims], Gt[f][4 cells][4], Xf[f] -> F[f][5]  (unit-level parity of jf_math.cuh)
+template <class T, int DIR>
+__global__ void face_flux_kernel(Gas<T> gas, const T* W, const T* Gt, const T* i24Xf, T* F, int nf) {
+  int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= nf) return;
+  const T* Wf = W + (size_t)f * 36;
+  const T* Gf = Gt + (size_t)f * 16;
+  auto w = [&](int m, int q) -> T { return Wf[(m + 2) * 6 + q]; };
+  auto g = [&](int m, int c) -> T { return Gf[(m + 1) * 4 + c]; };
+  T out[5];
+  if (gas.viscous) face_flux<T, DIR, true>(gas, w, g, i24Xf[f], out);
+  else face_flux<T, DIR, false>(gas, w, g, T(0), out);
+  for (int q = 0; q < 5; ++q) F[(size_t)f * 5 + q] = out[q];
+}
+
 // ------------------------------------------------------------------ diagnostics: ALU peak
 template <class T>
 __global__ void __launch_bounds__(256) alu_peak_kernel(T* out, int iters, T seed) {

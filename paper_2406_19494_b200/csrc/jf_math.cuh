@@ -17,7 +17,17 @@ namespace jf {
 template <class T> struct Num;
 template <> struct Num<double> {
   static __device__ __forceinline__ double sqrt_(double a) { return sqrt(a); }
-  static __device__ __forceinline__ double rcp(double a) { return 1.0 / a; }
+  static __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+  // reciprocal for normal, finite a: hardware seed (MUFU.RCP64H, ~2^-20) + two Newton steps
+  // (4 DFMA) => ~1 ulp, not correctly rounded; about half the issue slots of 1.0/a.
+  static __device__ __forceinline__ double rcp(double a) {
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+    double e = fma(-a, x, 1.0);
+    x = fma(x, e, x);
+    e = fma(-a, x, 1.0);
+    return fma(x, e, x);
+  }
   static __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
   static __device__ __forceinline__ double min_(double a, double b) { return fmin(a, b); }
   static __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
@@ -25,6 +35,7 @@ template <> struct Num<double> {
 };
 template <> struct Num<float> {
   static __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
+  static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
   static __device__ __forceinline__ float rcp(float a) { return 1.0f / a; }
   static __device__ __forceinline__ float rsqrt_(float a) { return 1.0f / sqrtf(a); }
   static __device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
@@ -61,24 +72,45 @@ __device__ __forceinline__ T viscosity(const Gas<T>& gas, T Tf) {
   return gas.mu_ref * (r * Num<T>::sqrt_(r)) * gas.TrefS * Num<T>::rcp(Tf + gas.S);
 }
 
-// WENO5-JS value at the face between v2 and v3; one division.
+// WENO5-JS left and right states at the face between s2 | s3 from the six cells s0..s5
+// (L: stencil s0..s4; R: mirrored stencil s5..s1).  Difference form:
+//   v = p1 + [w0 (p0-p1) + w2 (p2-p1)],  p0-p1 = (A0-A1)/3,  p2-p1 = (A1-A2)/6,
+// A_k the second differences (shared between L and R), weights as products of the other two
+// e_k = (beta_k+eps)^2 (one reciprocal each).  Smoothness indicators are carried as 4*beta
+// (eps scaled likewise), which leaves the weights unchanged.
 template <class T>
-__device__ __forceinline__ T weno5(T v0, T v1, T v2, T v3, T v4) {
-  const T eps = T(1e-6), c1312 = T(13.0 / 12.0);
-  T a0 = v0 - T(2) * v1 + v2, b0 = v0 - T(4) * v1 + T(3) * v2;
-  T a1 = v1 - T(2) * v2 + v3, b1 = v1 - v3;
-  T a2 = v2 - T(2) * v3 + v4, b2 = T(3) * v2 - T(4) * v3 + v4;
-  T e0 = c1312 * (a0 * a0) + T(0.25) * (b0 * b0) + eps;
-  T e1 = c1312 * (a1 * a1) + T(0.25) * (b1 * b1) + eps;
-  T e2 = c1312 * (a2 * a2) + T(0.25) * (b2 * b2) + eps;
-  e0 *= e0; e1 *= e1; e2 *= e2;
-  T n0 = T(0.1) * (e1 * e2), n1 = T(0.6) * (e0 * e2), n2 = T(0.3) * (e0 * e1);
-  T q0 = T(2) * v0 - T(7) * v1 + T(11) * v2;
-  T q1 = T(5) * v2 - v1 + T(2) * v3;
-  T q2 = T(2) * v2 + T(5) * v3 - v4;
-  T num = n0 * q0 + n1 * q1 + n2 * q2;
-  T den = T(6) * (n0 + n1 + n2);
-  return num / den;
+__device__ __forceinline__ void weno5_pair(T s0, T s1, T s2, T s3, T s4, T s5, T& vL, T& vR) {
+  using N = Num<T>;
+  const T eps4 = T(4e-6), c133 = T(13.0 / 3.0), sixth = T(1.0 / 6.0);
+  const T c30 = T(1.0 / 30.0), c20 = T(1.0 / 20.0);
+  T A0 = N::fma_(T(-2), s1, s0) + s2, A1 = N::fma_(T(-2), s2, s1) + s3;
+  T A2 = N::fma_(T(-2), s3, s2) + s4, A3 = N::fma_(T(-2), s4, s3) + s5;
+  T cA0 = c133 * A0, cA1 = c133 * A1, cA2 = c133 * A2, cA3 = c133 * A3;
+  T d01 = A0 - A1, d12 = A1 - A2, d23 = A2 - A3;
+  {  // left-biased
+    T b0 = N::fma_(T(3), s2, N::fma_(T(-4), s1, s0)), b1 = s1 - s3, b2 = N::fma_(T(3), s2, N::fma_(T(-4), s3, s4));
+    T e0 = N::fma_(cA0, A0, N::fma_(b0, b0, eps4));
+    T e1 = N::fma_(cA1, A1, N::fma_(b1, b1, eps4));
+    T e2 = N::fma_(cA2, A2, N::fma_(b2, b2, eps4));
+    e0 *= e0; e1 *= e1; e2 *= e2;
+    T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
+    T den = N::fma_(T(0.3), E01, N::fma_(T(0.6), E02, T(0.1) * E12));
+    T num = N::fma_(c30 * E12, d01, (c20 * E01) * d12);
+    T p1 = sixth * N::fma_(T(5), s2, N::fma_(T(2), s3, -s1));
+    vL = N::fma_(num, N::rcp(den), p1);
+  }
+  {  // right-biased: stencil (s5,s4,s3,s2,s1): A0' = A3, A1' = A2, A2' = A1
+    T b0 = N::fma_(T(3), s3, N::fma_(T(-4), s4, s5)), b1 = s4 - s2, b2 = N::fma_(T(3), s3, N::fma_(T(-4), s2, s1));
+    T e0 = N::fma_(cA3, A3, N::fma_(b0, b0, eps4));
+    T e1 = N::fma_(cA2, A2, N::fma_(b1, b1, eps4));
+    T e2 = N::fma_(cA1, A1, N::fma_(b2, b2, eps4));
+    e0 *= e0; e1 *= e1; e2 *= e2;
+    T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
+    T den = N::fma_(T(0.3), E01, N::fma_(T(0.6), E02, T(0.1) * E12));
+    T numn = N::fma_(c20 * E01, d12, (c30 * E12) * d23);     // A0'-A1' = -(A2-A3), A1'-A2' = -(A1-A2)
+    T p1 = sixth * N::fma_(T(5), s3, N::fma_(T(2), s2, -s4));
+    vR = N::fma_(-numn, N::rcp(den), p1);
+  }
 }
 
 // HLLC flux in the rotated frame: states (rho, un, ut1, ut2, p) -> F = [mass, n, t1, t2, energy]
@@ -99,7 +131,7 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
   T ct = N::sqrt_(gas.gm1 * (Ht - T(0.5) * (un * un + u1 * u1 + u2 * u2)));
   T SL = N::min_(L[1] - cL, un - ct), SR = N::max_(R[1] + cR, un + ct);
   T mL = L[0] * (SL - L[1]), mR = R[0] * (SR - R[1]);
-  T Ss = (R[4] - L[4] + L[1] * mL - R[1] * mR) / (mL - mR);
+  T Ss = (R[4] - L[4] + L[1] * mL - R[1] * mR) * N::rcp(mL - mR);
   // side selected by sign(S*)  (S* == 0: both star fluxes are mathematically equal)
   bool left = Ss >= T(0);
   T rho = left ? L[0] : R[0], vn = left ? L[1] : R[1], v1 = left ? L[2] : R[2], v2 = left ? L[3] : R[3];
@@ -133,8 +165,7 @@ __device__ __forceinline__ void face_flux(const Gas<T>& gas, const WAcc& w, cons
   for (int c = 0; c < 5; ++c) {
     const int q = qs[c];
     T s0 = w(-2, q), s1 = w(-1, q), s2 = w(0, q), s3 = w(1, q), s4 = w(2, q), s5 = w(3, q);
-    L[c] = weno5<T>(s0, s1, s2, s3, s4);
-    R[c] = weno5<T>(s5, s4, s3, s2, s1);
+    weno5_pair<T>(s0, s1, s2, s3, s4, s5, L[c], R[c]);
   }
   T Fr[5];
   hllc_rot<T>(gas, L, R, Fr);

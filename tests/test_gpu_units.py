@@ -1,0 +1,82 @@
+"""Unit-level GPU parity: the per-face arithmetic of the sweep kernels (jf_math.cuh, reached through
+jf_diag_face_flux of the C ABI) against the oracle's scheme functions on seeded random stencils."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+G, RG, PR = 1.4, 0.8, 0.72
+
+
+@pytest.fixture(scope="module")
+def jf():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2406_19494_b200 import binding
+    return binding
+
+
+def stencils(n, seed, jump=False):
+    rng = np.random.default_rng(seed)
+    W = np.empty((n, 6, 6))
+    base = rng.uniform(0.5, 2.0, (n, 1))
+    W[:, :, 0] = base + 0.2 * rng.uniform(-1, 1, (n, 6))
+    W[:, :, 1:4] = rng.uniform(-1.5, 1.5, (n, 1, 3)) + 0.3 * rng.uniform(-1, 1, (n, 6, 3))
+    W[:, :, 4] = rng.uniform(0.5, 3.0, (n, 1)) + 0.2 * rng.uniform(-1, 1, (n, 6))
+    if jump:                                   # discontinuity at a random position of the stencil
+        k = rng.integers(1, 6, n)
+        for f in range(n):
+            W[f, k[f]:, 0] *= 4.0
+            W[f, k[f]:, 4] *= 7.0
+            W[f, k[f]:, 1:4] += 2.0
+    W[:, :, 5] = W[:, :, 4] / (W[:, :, 0] * RG)
+    return W
+
+
+def oracle_face(ora, d, W, Gt, Xf, mu):
+    n, t1, t2 = d, (d + 1) % 3, (d + 2) % 3
+    WL = [ora.weno5(W[0:5, q]) for q in range(5)]
+    WR = [ora.weno5(W[5:0:-1, q]) for q in range(5)]
+    F = ora.hllc(d, G, WL, WR)
+    if mu["mu_ref"] > 0:
+        qs = [1 + n, 1 + t1, 1 + t2, 5]
+        dn = [ora.df(W[1:5, q], Xf) for q in qs]
+        fv = [ora.iface(W[1:5, q]) for q in qs]
+        gt = [ora.iface(Gt[:, c]) for c in range(4)]
+        m = ora.viscosity(mu, fv[3])
+        lam = m * G * RG / (G - 1) / PR
+        div = dn[0] + gt[1] + gt[3]
+        tnn, tn1, tn2 = m * (2 * dn[0] - 2.0 / 3.0 * div), m * (gt[0] + dn[1]), m * (gt[2] + dn[2])
+        F[1 + n] -= tnn
+        F[1 + t1] -= tn1
+        F[1 + t2] -= tn2
+        F[4] -= fv[0] * tnn + fv[1] * tn1 + fv[2] * tn2 + lam * dn[3]
+    return F
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+@pytest.mark.parametrize("kind", ["smooth", "jump", "viscous"])
+def test_face_flux_matches_oracle_functions(jf, ora, d, kind):
+    n = 300
+    W = stencils(n, seed=10 * d + len(kind), jump=(kind == "jump"))
+    rng = np.random.default_rng(5)
+    mu = {"sutherland": 1, "mu_ref": 0.05 if kind == "viscous" else 0.0, "T_ref": 1.0, "S": 0.4}
+    Gt = rng.uniform(-2, 2, (n, 4, 4))
+    Xf = rng.uniform(0.05, 0.2, n)
+    F = jf.jf_diag_face_flux("f64", d, G, RG, PR, mu, W, Gt, Xf)
+    Fo = np.array([oracle_face(ora, d, W[f], Gt[f], Xf[f], mu) for f in range(n)])
+    scale = np.maximum(np.max(np.abs(Fo), axis=1, keepdims=True), 1.0)
+    assert np.max(np.abs(F - Fo) / scale) <= 5e-14
+    F32 = jf.jf_diag_face_flux("f32", d, G, RG, PR, mu, W, Gt, Xf)
+    assert np.max(np.abs(F32 - Fo) / scale) <= 2e-5
+
+
+def test_face_flux_consistency_on_uniform_stencils(jf, ora):
+    # F(W,W) = F^c(W) (Eq. 3) to round-off on the GPU as well
+    rng = np.random.default_rng(3)
+    n = 64
+    W = np.repeat(stencils(n, 1)[:, :1, :], 6, axis=1)
+    mu = {"sutherland": 0, "mu_ref": 0.0, "T_ref": 1.0, "S": 0.0}
+    for d in range(3):
+        F = jf.jf_diag_face_flux("f64", d, G, RG, PR, mu, W)
+        Fo = np.array([ora.flux_phys(d, G, W[f, 0, :5]) for f in range(n)])
+        assert np.max(np.abs(F - Fo) / np.maximum(np.abs(Fo).max(axis=1, keepdims=True), 1)) <= 1e-14
