@@ -273,10 +273,10 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
   {
     Timed t(s, K_SWEEP_X);
     const int rows = P.n[1] * P.n[2];
-    const size_t sh = (size_t)jf::XS_WARPS * 6 * 64 * sizeof(T);
+    const size_t sh = (size_t)jf::XS_WARPS * jf::XS<VISC>::NV * jf::XS_RING * sizeof(T);
     jf::sweep_x_kernel<T, VISC><<<(rows + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
-  const size_t sh = (size_t)6 * 6 * jf::YZ_TX * jf::YZ_TY * sizeof(T);
+  const size_t sh = (size_t)jf::YZ_RING * jf::YZ<VISC>::NV * jf::YZ_TX * jf::YZ_TY * sizeof(T);
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
   jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0)};
   {
@@ -295,6 +295,21 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
   s->launches += 3;
   JF_CUDA(s, cudaPeekAtLastError());
   return JF_OK;
+}
+
+// The viscous y/z sweeps keep a 5-cell window of 10 values per thread in shared memory (50 KB per
+// 128-thread block in fp64): above the 48 KB default, so opt in once per solver.
+template <class T, bool VISC>
+cudaError_t opt_in_smem() {
+  const int sh = (int)((size_t)jf::YZ_RING * jf::YZ<VISC>::NV * jf::YZ_TX * jf::YZ_TY * sizeof(T));
+  cudaError_t e = cudaSuccess;
+  auto set = [&](const void* f) {
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
+  };
+  set((const void*)jf::sweep_yz_kernel<T, 1, VISC, 0>);
+  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 1>);
+  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 2>);
+  return e;
 }
 
 template <class T>
@@ -386,6 +401,11 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
                      ? setup<double>(s, s->d, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev)
                      : setup<float>(s, s->f, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev);
   if (st != JF_OK) { delete s; return st; }
+  {
+    cudaError_t ce = dtype == JF_F64 ? (s->viscous ? opt_in_smem<double, true>() : opt_in_smem<double, false>())
+                                     : (s->viscous ? opt_in_smem<float, true>() : opt_in_smem<float, false>());
+    if (ce != cudaSuccess) { delete s; return JF_ECUDA; }
+  }
   const int n[3] = {g->nx, g->ny, g->nz};
   s->seg_len[0] = 0;
   s->seg_len[1] = pick_segment((long long)n[0] * n[2], n[1]);

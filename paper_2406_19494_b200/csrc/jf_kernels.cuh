@@ -152,82 +152,108 @@ struct RKArgs {
 
 // ------------------------------------------------------------------ x sweep
 // One warp per (j,k) line.  Iteration kc loads padded cells [32kc, 32kc+32) (prefetched one
-// iteration ahead), converts them to primitives in a 64-cell warp-private ring, then evaluates
-// the 32 faces fi = 32kc-6+lane (face between padded cells fi+2 | fi+3) and writes
-// R = -(F_fi - F_{fi-1})/dx for cell fi-1; F_{fi-1} comes from the neighbouring lane (lane 0:
-// carried from the previous iteration).  R is written, not accumulated: the x sweep runs first.
-constexpr int XS_WARPS = 8;
+// iteration ahead), converts them to primitives in a 64-cell warp-private ring, then lane l does
+// the per-cell WENO of padded cell pc = 32kc-2+l (W^-_{pc+1/2}, W^+_{pc-1/2}), takes W^-_{pc-1/2}
+// from lane l-1, evaluates the face pc-1/2 (HLLC + dissipative flux) and writes
+// R = -(F_{pc-1/2} - F_{pc-3/2})/dx for cell pc-1 (F_{pc-3/2} from lane l-1; lane 0: carried from
+// the previous iteration).  R is written, not accumulated: the x sweep runs first.
+constexpr int XS_WARPS = 8, XS_RING = 64;
+template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, bool VISC>
 __global__ void __launch_bounds__(XS_WARPS * 32)
 sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* __restrict__ R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* ring_all = reinterpret_cast<T*>(smem_raw);
+  constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_y v, d_z u, d_z w]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row = blockIdx.x * XS_WARPS + warp;
   const int ny = P.n[1], nz = P.n[2], nx = P.n[0], Px = P.P[0];
   if (row >= ny * nz) return;
   const int j = row % ny, k = row / ny;
   const long long base = (long long)(k + NH) * P.sz + (long long)(j + NH) * P.sy;
-  T* ring = ring_all + warp * (6 * 64);
+  T* ring = reinterpret_cast<T*>(smem_raw) + warp * (NV * XS_RING);
   const Gas<T> gas = P.gas;
-  const T* g0 = G + (long long)(3 * 1 + 0) * P.vol + base;  // d_y u
-  const T* g1 = G + (long long)(3 * 1 + 1) * P.vol + base;  // d_y v
-  const T* g2 = G + (long long)(3 * 2 + 0) * P.vol + base;  // d_z u
-  const T* g3 = G + (long long)(3 * 2 + 2) * P.vol + base;  // d_z w
-  const int kmax = (nx + 6) / 32;
-  T raw[5];
-  {
-    const int p = lane;
+  const T* gsrc[4] = {G + (long long)(3 * 1 + 0) * P.vol + base, G + (long long)(3 * 1 + 1) * P.vol + base,
+                      G + (long long)(3 * 2 + 0) * P.vol + base, G + (long long)(3 * 2 + 2) * P.vol + base};
+  const int kmax = (nx + 5) / 32;            // last cell to treat: pc = nx+3
+  const unsigned full = 0xffffffffu;
+  const int src_lane = (lane + 31) & 31;
+  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
+  auto fetch = [&](int p) {
 #pragma unroll
     for (int q = 0; q < 5; ++q) raw[q] = (p < Px) ? U[q * P.vol + base + p] : T(1);
-  }
-  T carry[5] = {T(0), T(0), T(0), T(0), T(0)};
+    if (VISC) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) gn[c] = (p < Px) ? gsrc[c][p] : T(0);
+    }
+  };
+  fetch(lane);
+  T WmOld[5], Fold[5];                       // this lane's W^- and F of the previous iteration
+#pragma unroll
+  for (int q = 0; q < 5; ++q) { WmOld[q] = T(1); Fold[q] = T(0); }
   for (int kc = 0; kc <= kmax; ++kc) {
     const int p = 32 * kc + lane;
     if (p < Px) {
       T W[6];
       cons_to_prim<T>(gas, raw[0], raw[1], raw[2], raw[3], raw[4], W);
+      T* dst = ring + (p & (XS_RING - 1));
 #pragma unroll
-      for (int q = 0; q < 6; ++q) ring[q * 64 + (p & 63)] = W[q];
-    }
-    if (kc < kmax) {
-      const int pn = p + 32;
+      for (int q = 0; q < 5; ++q) dst[q * XS_RING] = W[q];
+      if (VISC) {
+        dst[5 * XS_RING] = W[5];
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raw[q] = (pn < Px) ? U[q * P.vol + base + pn] : T(1);
+        for (int c = 0; c < 4; ++c) dst[(6 + c) * XS_RING] = gn[c];
+      }
     }
+    if (kc < kmax) fetch(p + 32);
     __syncwarp();
-    const int fi = 32 * kc - 6 + lane;
-    const int pc = fi + 2;  // padded index of the cell on the low side of the face
-    T F[5] = {T(0), T(0), T(0), T(0), T(0)};
-    if (fi >= 0 && fi <= nx) {
-      auto w = [&](int m, int q) -> T { return ring[q * 64 + ((pc + m) & 63)]; };
-      auto g = [&](int m, int c) -> T {
-        const T* gp = c == 0 ? g0 : (c == 1 ? g1 : (c == 2 ? g2 : g3));
-        return __ldg(gp + pc + m);
-      };
-      face_flux<T, 0, VISC>(gas, w, g, VISC ? P.i24Xf[0][pc] : T(0), F);
-    }
+    const int pc = 32 * kc - 2 + lane;
+    auto w = [&](int m, int q) -> T { return ring[q * XS_RING + ((pc + m) & (XS_RING - 1))]; };
+    auto g = [&](int m, int c) -> T { return ring[(6 + c) * XS_RING + ((pc + m) & (XS_RING - 1))]; };
+    T Wm[5], Wp[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Wm[q] = T(1); Wp[q] = T(1); }
+    if (pc >= 2 && pc <= nx + 3) weno_cell_states<T, 0>(w, Wm, Wp);
+    // W^-_{pc-1/2} comes from lane-1; lane 0 takes lane 31's value of the previous iteration
+    T WL[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      T Fm = __shfl_up_sync(0xffffffffu, F[q], 1);
-      if (lane == 0) Fm = carry[q];
-      carry[q] = __shfl_sync(0xffffffffu, F[q], 31);
-      if (fi >= 1 && fi <= nx) R[q * P.vol + base + pc] = -(F[q] - Fm) * P.inv_dl[0][pc];
+      WL[q] = __shfl_sync(full, lane == 31 ? WmOld[q] : Wm[q], src_lane);
+      WmOld[q] = Wm[q];
+    }
+    T F[5] = {T(0), T(0), T(0), T(0), T(0)};
+    if (pc >= 3 && pc <= nx + 3)
+      face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][pc - 1] : T(0), F);
+    const T idl = (pc >= 4 && pc <= nx + 3) ? P.inv_dl[0][pc - 1] : T(0);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      T Fm = __shfl_sync(full, lane == 31 ? Fold[q] : F[q], src_lane);
+      Fold[q] = F[q];
+      if (pc >= 4 && pc <= nx + 3) R[q * P.vol + base + pc - 1] = -(F[q] - Fm) * idl;
     }
     __syncwarp();
   }
 }
 
 // ------------------------------------------------------------------ y / z sweeps (+ RK3 stage)
+// One thread per (x, other) column marching along DIR over the segment [c0, c1) (warp = 32
+// consecutive x: every access coalesced).  A thread-private shared-memory ring holds the window
+// c-2..c+2 of primitives (and of the four transverse centre derivatives).  Step c: per-cell WENO
+// of cell c (W^-_{c+1/2}, W^+_{c-1/2}); face c-1/2 from the carried W^-_{c-1/2} and W^+_{c-1/2};
+// update of cell c-1 with F_{c-1/2} - F_{c-3/2}.  The loads of the next window cell and of the
+// arrays the update needs are issued after the WENO part and consumed after the face flux.
 // MODE 0: R -= dF/Delta (accumulate).  MODE 1: R = R - dF/Delta + S (final R of Eq. 6).
 // MODE 2: as 1, then the SSP-RK3 stage update U_out = a U^n + b (U_s + dt R) (R not stored).
-constexpr int YZ_TX = 32, YZ_TY = 4;
+#ifndef JF_YZ_MINB
+#define JF_YZ_MINB 3
+#endif
+constexpr int YZ_TX = 32, YZ_TY = 4, YZ_RING = 5;
+template <bool VISC> struct YZ { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, int DIR, bool VISC, int MODE>
-__global__ void __launch_bounds__(YZ_TX * YZ_TY)
+__global__ void __launch_bounds__(YZ_TX * YZ_TY, JF_YZ_MINB)
 sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* R, RKArgs<T> rk, int L) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* ring = reinterpret_cast<T*>(smem_raw);  // [6 slots][6 vars][threads]
-  constexpr int NT = YZ_TX * YZ_TY;
+  T* ring = reinterpret_cast<T*>(smem_raw);  // [5 slots][NV][threads]
+  constexpr int NT = YZ_TX * YZ_TY, NV = YZ<VISC>::NV;
   constexpr int OTH = (DIR == 1) ? 2 : 1;    // the non-marching, non-x axis
   const int tid = threadIdx.y * YZ_TX + threadIdx.x;
   const int ix = blockIdx.x * YZ_TX + threadIdx.x;
@@ -239,69 +265,99 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   const int c0 = blockIdx.z * L, c1 = min(c0 + L, N);
   const Gas<T> gas = P.gas;
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  const T* g0 = G + (long long)(3 * t1 + n) * P.vol + col;
-  const T* g1 = G + (long long)(3 * t1 + t1) * P.vol + col;
-  const T* g2 = G + (long long)(3 * t2 + n) * P.vol + col;
-  const T* g3 = G + (long long)(3 * t2 + t2) * P.vol + col;
-  auto put = [&](int pm, const T raw[5]) {
+  const T* gsrc[4] = {G + (long long)(3 * t1 + n) * P.vol + col, G + (long long)(3 * t1 + t1) * P.vol + col,
+                      G + (long long)(3 * t2 + n) * P.vol + col, G + (long long)(3 * t2 + t2) * P.vol + col};
+  T* mine = ring + tid;
+  auto put = [&](int slot, const T raw[5], const T gn[4]) {
     T W[6];
     cons_to_prim<T>(gas, raw[0], raw[1], raw[2], raw[3], raw[4], W);
-    const int slot = pm % 6;
+    T* dst = mine + slot * (NV * NT);
 #pragma unroll
-    for (int q = 0; q < 6; ++q) ring[(slot * 6 + q) * NT + tid] = W[q];
+    for (int q = 0; q < 5; ++q) dst[q * NT] = W[q];
+    if (VISC) {
+      dst[5 * NT] = W[5];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) dst[(6 + c) * NT] = gn[c];
+    }
   };
-  T raw[5];
-  for (int pm = c0; pm < c0 + 6; ++pm) {  // padded cells c0 .. c0+5  (= cells c0-3 .. c0+2)
+  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
+  // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots 0..4
+  for (int s = 0; s < YZ_RING; ++s) {
+    const long long o = col + (long long)(c0 + s) * sm;
 #pragma unroll
-    for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + col + pm * sm];
-    put(pm, raw);
+    for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + o];
+    if (VISC) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) gn[c] = gsrc[c][(long long)(c0 + s) * sm];
+    }
+    put(s, raw, gn);
   }
-  T Fprev[5] = {T(0), T(0), T(0), T(0), T(0)};
-  for (int f = c0 - 1; f < c1; ++f) {      // face on the high side of cell f
-    const int pf = f + NH;
-    const bool more = f + 1 < c1;
-    if (more) {
+  T WmPrev[5], Fprev[5];
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + col + (long long)(pf + 4) * sm];
-    }
-    int slot[6];
+  for (int q = 0; q < 5; ++q) { WmPrev[q] = T(1); Fprev[q] = T(0); }
+  int s0 = 0;                                // slot of cell c-2
+  for (int c = c0 - 1; c <= c1; ++c) {
+    const int pc = c + NH;
+    int slot[YZ_RING];
     {
-      int s = (pf - 2) % 6;
+      int s = s0;
 #pragma unroll
-      for (int m = 0; m < 6; ++m) { slot[m] = s; s = (s == 5) ? 0 : s + 1; }
+      for (int m = 0; m < YZ_RING; ++m) { slot[m] = s * (NV * NT); s = (s == YZ_RING - 1) ? 0 : s + 1; }
     }
-    auto w = [&](int m, int q) -> T { return ring[(slot[m + 2] * 6 + q) * NT + tid]; };
-    auto g = [&](int m, int c) -> T {
-      const T* gp = c == 0 ? g0 : (c == 1 ? g1 : (c == 2 ? g2 : g3));
-      return __ldg(gp + (long long)(pf + m) * sm);
-    };
-    T F[5];
-    face_flux<T, DIR, VISC>(gas, w, g, VISC ? P.i24Xf[DIR][pf] : T(0), F);
-    if (f >= c0) {
-      const long long o = col + (long long)pf * sm;
-      const T idl = P.inv_dl[DIR][pf];
-      T Rv[5];
+    auto w = [&](int m, int q) -> T { return mine[slot[m + 2] + q * NT]; };
+    auto g = [&](int m, int cc) -> T { return mine[slot[m + 2] + (6 + cc) * NT]; };
+    T Wm[5], Wp[5];
+    weno_cell_states<T, DIR>(w, Wm, Wp);
+    // issue the loads this step consumes at its end
+    const bool more = c < c1;                // another cell follows: its window needs padded pc+3
+    const bool upd = c > c0;                 // cell c-1 is in [c0, c1): update it
+    const long long o = col + (long long)(pc - 1) * sm;
+    T Rold[5], un[5], us[5];
+    if (more) {
+      const long long on = col + (long long)(pc + 3) * sm;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) Rv[q] = R[q * P.vol + o] - (F[q] - Fprev[q]) * idl;
-      if (MODE >= 1) {
-        T rho = w(0, 0), u = w(0, 1), v = w(0, 2), ww = w(0, 3);
-        Rv[1] += rho * gas.g[0]; Rv[2] += rho * gas.g[1]; Rv[3] += rho * gas.g[2];
-        Rv[4] += rho * (u * gas.g[0] + v * gas.g[1] + ww * gas.g[2]);
+      for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + on];
+      if (VISC) {
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) gn[cc] = gsrc[cc][(long long)(pc + 3) * sm];
       }
+    }
+    if (upd) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Rold[q] = R[q * P.vol + o];
       if (MODE == 2) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          T un = rk.Un[q * P.vol + o], us = U[q * P.vol + o];
-          rk.Uout[q * P.vol + o] = rk.a * un + rk.b * (us + rk.dt * Rv[q]);
-        }
-      } else {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) R[q * P.vol + o] = Rv[q];
+        for (int q = 0; q < 5; ++q) { un[q] = rk.Un[q * P.vol + o]; us[q] = U[q * P.vol + o]; }
       }
     }
+    if (c >= c0) {                           // face c-1/2
+      T F[5];
+      face_flux<T, DIR, VISC>(gas, WmPrev, Wp, w, g, VISC ? P.i24Xf[DIR][pc - 1] : T(0), F);
+      if (upd) {
+        const T idl = P.inv_dl[DIR][pc - 1];
+        T Rv[5];
 #pragma unroll
-    for (int q = 0; q < 5; ++q) Fprev[q] = F[q];
-    if (more) put(pf + 4, raw);
+        for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - Fprev[q]) * idl;
+        if (MODE >= 1) {
+          T rho = w(-1, 0), u = w(-1, 1), v = w(-1, 2), ww = w(-1, 3);
+          Rv[1] += rho * gas.g[0]; Rv[2] += rho * gas.g[1]; Rv[3] += rho * gas.g[2];
+          Rv[4] += rho * (u * gas.g[0] + v * gas.g[1] + ww * gas.g[2]);
+        }
+        if (MODE == 2) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) rk.Uout[q * P.vol + o] = rk.a * un[q] + rk.b * (us[q] + rk.dt * Rv[q]);
+        } else {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) R[q * P.vol + o] = Rv[q];
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Fprev[q] = F[q];
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) WmPrev[q] = Wm[q];
+    if (more) put(s0, raw, gn);              // cell c+3 replaces cell c-2
+    s0 = (s0 == YZ_RING - 1) ? 0 : s0 + 1;
   }
 }
 
@@ -372,18 +428,24 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
 }
 
 // ------------------------------------------------------------------ diagnostics: one face flux per thread
-// W[f][6 cells][6 prims], Gt[f][4 cells][4], Xf[f] -> F[f][5]  (unit-level parity of jf_math.cuh)
+// W[f][6 cells][6 prims] (cells i-2..i+3), Gt[f][4 cells][4] (cells i-1..i+2), Xf[f] -> F[f][5] of
+// the face i+1/2: per-cell WENO of cell i (W^-) and of cell i+1 (W^+), then the face flux —
+// the same device functions the sweeps call (unit-level parity of jf_math.cuh).
 template <class T, int DIR>
 __global__ void face_flux_kernel(Gas<T> gas, const T* W, const T* Gt, const T* i24Xf, T* F, int nf) {
   int f = blockIdx.x * blockDim.x + threadIdx.x;
   if (f >= nf) return;
   const T* Wf = W + (size_t)f * 36;
   const T* Gf = Gt + (size_t)f * 16;
-  auto w = [&](int m, int q) -> T { return Wf[(m + 2) * 6 + q]; };
-  auto g = [&](int m, int c) -> T { return Gf[(m + 1) * 4 + c]; };
+  auto w0 = [&](int m, int q) -> T { return Wf[(m + 2) * 6 + q]; };   // offsets about cell i
+  auto w1 = [&](int m, int q) -> T { return Wf[(m + 3) * 6 + q]; };   // offsets about cell i+1
+  auto g1 = [&](int m, int c) -> T { return Gf[(m + 2) * 4 + c]; };   // offsets about cell i+1
+  T WmL[5], WpL[5], WmR[5], WpR[5];
+  weno_cell_states<T, DIR>(w0, WmL, WpL);
+  weno_cell_states<T, DIR>(w1, WmR, WpR);
   T out[5];
-  if (gas.viscous) face_flux<T, DIR, true>(gas, w, g, i24Xf[f], out);
-  else face_flux<T, DIR, false>(gas, w, g, T(0), out);
+  if (gas.viscous) face_flux<T, DIR, true>(gas, WmL, WpR, w1, g1, i24Xf[f], out);
+  else face_flux<T, DIR, false>(gas, WmL, WpR, w1, g1, T(0), out);
   for (int q = 0; q < 5; ++q) F[(size_t)f * 5 + q] = out[q];
 }
 

@@ -4,8 +4,13 @@
 // cores): the formulas of DESIGN.md "Readings" (WENO5-JS, HLLC with Roe-average wave speeds,
 // 4th-order central dissipative flux, Sutherland) restructured to cut divisions — the FP64
 // pipe pays ~10 issue slots per division:
-//   * WENO5: the three non-linear weights are formed as products n_k = d_k e_l e_m with
-//     e_k = (beta_k + eps)^2, so one reconstruction costs ONE division instead of four;
+//   * WENO5 is evaluated per CELL, not per face: the left-biased state at face i+1/2 and the
+//     right-biased state at face i-1/2 are both built from cells i-2..i+2 with the SAME three
+//     smoothness indicators (the mirrored stencil of Jiang & Shu only swaps beta_0 and beta_2
+//     and the linear weights), so the indicators are computed once for two reconstructions;
+//   * the three non-linear weights are formed as products n_k = d_k e_l e_m with
+//     e_k = (beta_k + eps)^2, so one reconstruction costs ONE reciprocal instead of four
+//     divisions; reciprocal / square roots are a hardware seed plus one cubic Newton step;
 //   * HLLC: only the star state on the side selected by sign(S*) is evaluated (the other is
 //     multiplied by an exact zero in the closed form), reciprocals are shared.
 // Results agree with the closed forms to a few ulp, not bit-wise (tolerance: DESIGN.md).
@@ -16,19 +21,25 @@ namespace jf {
 
 template <class T> struct Num;
 template <> struct Num<double> {
-  static __device__ __forceinline__ double sqrt_(double a) { return sqrt(a); }
   static __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
-  // reciprocal for normal, finite a: hardware seed (MUFU.RCP64H, ~2^-20) + two Newton steps
-  // (4 DFMA) => ~1 ulp, not correctly rounded; about half the issue slots of 1.0/a.
+  // reciprocal for normal, finite a: hardware seed (MUFU.RCP64H, rel. error <= 2^-23) and one
+  // cubic step x (1 + e + e^2), e = 1 - a x  =>  error ~ e^3 < 2^-66: a few ulp-fractions, not
+  // correctly rounded; 3 DFMA instead of the ~10-instruction 1.0/a.
   static __device__ __forceinline__ double rcp(double a) {
     double x;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
     double e = fma(-a, x, 1.0);
-    x = fma(x, e, x);
-    e = fma(-a, x, 1.0);
-    return fma(x, e, x);
+    return fma(x, fma(e, e, e), x);
   }
-  static __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
+  // 1/sqrt(a), normal finite a > 0: seed (MUFU.RSQ64H) and one cubic step
+  // y (1 + e/2 + 3 e^2/8), e = 1 - a y^2.
+  static __device__ __forceinline__ double rsqrt_(double a) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double e = fma(-(a * y), y, 1.0);
+    return fma(y, e * fma(0.375, e, 0.5), y);
+  }
+  static __device__ __forceinline__ double sqrt_(double a) { return a * rsqrt_(a); }
   static __device__ __forceinline__ double min_(double a, double b) { return fmin(a, b); }
   static __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
   static __device__ __forceinline__ double abs_(double a) { return fabs(a); }
@@ -72,44 +83,40 @@ __device__ __forceinline__ T viscosity(const Gas<T>& gas, T Tf) {
   return gas.mu_ref * (r * Num<T>::sqrt_(r)) * gas.TrefS * Num<T>::rcp(Tf + gas.S);
 }
 
-// WENO5-JS left and right states at the face between s2 | s3 from the six cells s0..s5
-// (L: stencil s0..s4; R: mirrored stencil s5..s1).  Difference form:
-//   v = p1 + [w0 (p0-p1) + w2 (p2-p1)],  p0-p1 = (A0-A1)/3,  p2-p1 = (A1-A2)/6,
-// A_k the second differences (shared between L and R), weights as products of the other two
-// e_k = (beta_k+eps)^2 (one reciprocal each).  Smoothness indicators are carried as 4*beta
-// (eps scaled likewise), which leaves the weights unchanged.
+// WENO5-JS, per cell: from the five cells (a,b,c,d,e) = v_{i-2..i+2} form
+//   vm = W^-_{i+1/2}: the left-biased value at face i+1/2  = weno(a,b,c,d,e) of the definition,
+//   vp = W^+_{i-1/2}: the right-biased value at face i-1/2 = weno(e,d,c,b,a).
+// Both use the same smoothness indicators beta_0(a,b,c), beta_1(b,c,d), beta_2(c,d,e): the
+// mirrored stencil swaps beta_0 <-> beta_2 and the linear weights (1,6,3)/10 <-> (3,6,1)/10.
+// Difference form: v = p1 + [w0 (p0-p1) + w2 (p2-p1)] / sum, with second differences A_k,
+//   vm: p0-p1 = (A0-A1)/3, p2-p1 = (A1-A2)/6;   vp: p0'-p1' = -(A1-A2)/3, p2'-p1' = -(A0-A1)/6,
+// weights as products of the other two e_k = (beta_k+eps)^2 (one reciprocal per value).
+// Indicators are carried as 4*beta (eps scaled likewise), which leaves the weights unchanged.
 template <class T>
-__device__ __forceinline__ void weno5_pair(T s0, T s1, T s2, T s3, T s4, T s5, T& vL, T& vR) {
+__device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp) {
   using N = Num<T>;
   const T eps4 = T(4e-6), c133 = T(13.0 / 3.0), sixth = T(1.0 / 6.0);
   const T c30 = T(1.0 / 30.0), c20 = T(1.0 / 20.0);
-  T A0 = N::fma_(T(-2), s1, s0) + s2, A1 = N::fma_(T(-2), s2, s1) + s3;
-  T A2 = N::fma_(T(-2), s3, s2) + s4, A3 = N::fma_(T(-2), s4, s3) + s5;
-  T cA0 = c133 * A0, cA1 = c133 * A1, cA2 = c133 * A2, cA3 = c133 * A3;
-  T d01 = A0 - A1, d12 = A1 - A2, d23 = A2 - A3;
-  {  // left-biased
-    T b0 = N::fma_(T(3), s2, N::fma_(T(-4), s1, s0)), b1 = s1 - s3, b2 = N::fma_(T(3), s2, N::fma_(T(-4), s3, s4));
-    T e0 = N::fma_(cA0, A0, N::fma_(b0, b0, eps4));
-    T e1 = N::fma_(cA1, A1, N::fma_(b1, b1, eps4));
-    T e2 = N::fma_(cA2, A2, N::fma_(b2, b2, eps4));
-    e0 *= e0; e1 *= e1; e2 *= e2;
-    T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
-    T den = N::fma_(T(0.3), E01, N::fma_(T(0.6), E02, T(0.1) * E12));
-    T num = N::fma_(c30 * E12, d01, (c20 * E01) * d12);
-    T p1 = sixth * N::fma_(T(5), s2, N::fma_(T(2), s3, -s1));
-    vL = N::fma_(num, N::rcp(den), p1);
+  T A0 = N::fma_(T(-2), b, a) + c, A1 = N::fma_(T(-2), c, b) + d, A2 = N::fma_(T(-2), d, c) + e;
+  T b0 = N::fma_(T(3), c, N::fma_(T(-4), b, a)), b1 = b - d, b2 = N::fma_(T(3), c, N::fma_(T(-4), d, e));
+  T e0 = N::fma_(c133 * A0, A0, N::fma_(b0, b0, eps4));
+  T e1 = N::fma_(c133 * A1, A1, N::fma_(b1, b1, eps4));
+  T e2 = N::fma_(c133 * A2, A2, N::fma_(b2, b2, eps4));
+  e0 *= e0; e1 *= e1; e2 *= e2;
+  T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
+  T t1 = E12 * (A0 - A1), t2 = E01 * (A1 - A2);
+  T mid = T(0.6) * E02;
+  {  // face i+1/2: weights (0.1 E12, 0.6 E02, 0.3 E01)
+    T den = N::fma_(T(0.3), E01, N::fma_(T(0.1), E12, mid));
+    T num = N::fma_(c30, t1, c20 * t2);
+    T p1 = sixth * N::fma_(T(5), c, N::fma_(T(2), d, -b));
+    vm = N::fma_(num, N::rcp(den), p1);
   }
-  {  // right-biased: stencil (s5,s4,s3,s2,s1): A0' = A3, A1' = A2, A2' = A1
-    T b0 = N::fma_(T(3), s3, N::fma_(T(-4), s4, s5)), b1 = s4 - s2, b2 = N::fma_(T(3), s3, N::fma_(T(-4), s2, s1));
-    T e0 = N::fma_(cA3, A3, N::fma_(b0, b0, eps4));
-    T e1 = N::fma_(cA2, A2, N::fma_(b1, b1, eps4));
-    T e2 = N::fma_(cA1, A1, N::fma_(b2, b2, eps4));
-    e0 *= e0; e1 *= e1; e2 *= e2;
-    T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
-    T den = N::fma_(T(0.3), E01, N::fma_(T(0.6), E02, T(0.1) * E12));
-    T numn = N::fma_(c20 * E01, d12, (c30 * E12) * d23);     // A0'-A1' = -(A2-A3), A1'-A2' = -(A1-A2)
-    T p1 = sixth * N::fma_(T(5), s3, N::fma_(T(2), s2, -s4));
-    vR = N::fma_(-numn, N::rcp(den), p1);
+  {  // face i-1/2: weights (0.3 E12, 0.6 E02, 0.1 E01)
+    T den = N::fma_(T(0.1), E01, N::fma_(T(0.3), E12, mid));
+    T num = N::fma_(c20, t1, c30 * t2);
+    T p1 = sixth * N::fma_(T(5), c, N::fma_(T(2), b, -d));
+    vp = N::fma_(-num, N::rcp(den), p1);
   }
 }
 
@@ -151,46 +158,64 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
   F[4] = F4 + Sc * (Es - E);
 }
 
-// Total face flux (convective - dissipative, Eq. 6) of the face between cells 0 and +1 along DIR.
-//   w(m, q): primitive q in {rho,u,v,w,p,T} of the cell at offset m in -2..3 along DIR
-//   g(m, c): transverse centre derivatives at offset m in -1..2:
+// Dissipative flux (Eq. 4-5, rotated frame) of the face between cells -1 | 0 along DIR, subtracted
+// from Fr = [mass, n, t1, t2, energy].
+//   w(m, q): primitive q in {rho,u,v,w,p,T} of the cell at offset m in -2..1 along DIR
+//   g(m, c): transverse centre derivatives at offset m in -2..1:
 //            c = 0: d_t1 u_n, 1: d_t1 u_t1, 2: d_t2 u_n, 3: d_t2 u_t2
 //   i24Xf: 1/(24 X_xi^f) of this face.   (n,t1,t2) = (DIR, DIR+1, DIR+2) mod 3.
-template <class T, int DIR, bool VISC, class WAcc, class GAcc>
-__device__ __forceinline__ void face_flux(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T F[5]) {
+template <class T, int DIR, class WAcc, class GAcc>
+__device__ __forceinline__ void viscous_sub(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T Fr[5]) {
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  constexpr int qs[5] = {0, 1 + n, 1 + t1, 1 + t2, 4};
-  T L[5], R[5];
+  T dn[4], fv[4];  // normal derivative and face value of u_n, u_t1, u_t2, T
+  constexpr int qv[4] = {1 + n, 1 + t1, 1 + t2, 5};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    T m1 = w(-2, qv[c]), c0 = w(-1, qv[c]), p1 = w(0, qv[c]), p2 = w(1, qv[c]);
+    dn[c] = (T(27) * (p1 - c0) - (p2 - m1)) * i24Xf;
+    fv[c] = (T(9) * (c0 + p1) - (m1 + p2)) * T(1.0 / 16.0);
+  }
+  T gt[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+    gt[c] = (T(9) * (g(-1, c) + g(0, c)) - (g(-2, c) + g(1, c))) * T(1.0 / 16.0);
+  T mu = viscosity<T>(gas, fv[3]);
+  T div = dn[0] + gt[1] + gt[3];
+  T tnn = mu * (T(2) * dn[0] - T(2.0 / 3.0) * div);
+  T tn1 = mu * (gt[0] + dn[1]);
+  T tn2 = mu * (gt[2] + dn[2]);
+  Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
+  Fr[4] -= fv[0] * tnn + fv[1] * tn1 + fv[2] * tn2 + mu * gas.lam_fac * dn[3];
+}
+
+// Rotated-frame component order of direction DIR: slot c of (rho, u_n, u_t1, u_t2, p) is
+// primitive / conservative index rot_q<DIR>(c).
+template <int DIR>
+__device__ __forceinline__ constexpr int rot_q(int c) {
+  return c == 0 ? 0 : (c == 4 ? 4 : 1 + (DIR + c - 1) % 3);
+}
+
+// Per-cell WENO of the five primitives of the cell at offset 0 (window -2..2 through w), in
+// rotated order: Wm = W^-_{+1/2}, Wp = W^+_{-1/2}.
+template <class T, int DIR, class WAcc>
+__device__ __forceinline__ void weno_cell_states(const WAcc& w, T Wm[5], T Wp[5]) {
 #pragma unroll
   for (int c = 0; c < 5; ++c) {
-    const int q = qs[c];
-    T s0 = w(-2, q), s1 = w(-1, q), s2 = w(0, q), s3 = w(1, q), s4 = w(2, q), s5 = w(3, q);
-    weno5_pair<T>(s0, s1, s2, s3, s4, s5, L[c], R[c]);
+    const int q = rot_q<DIR>(c);
+    weno5_cell<T>(w(-2, q), w(-1, q), w(0, q), w(1, q), w(2, q), Wm[c], Wp[c]);
   }
+}
+
+// Total face flux F = F^c - F^d (Eq. 6) of the face between cells -1 | 0 from its rotated
+// left / right states; un-rotated into (rho, rho u, rho v, rho w, E) slots.
+template <class T, int DIR, bool VISC, class WAcc, class GAcc>
+__device__ __forceinline__ void face_flux(const Gas<T>& gas, const T WL[5], const T WR[5], const WAcc& w,
+                                          const GAcc& g, T i24Xf, T F[5]) {
   T Fr[5];
-  hllc_rot<T>(gas, L, R, Fr);
-  if (VISC) {
-    T dn[4], fv[4];  // normal derivative and face value of u_n, u_t1, u_t2, T
-    constexpr int qv[4] = {1 + n, 1 + t1, 1 + t2, 5};
+  hllc_rot<T>(gas, WL, WR, Fr);
+  if (VISC) viscous_sub<T, DIR>(gas, w, g, i24Xf, Fr);
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      T m1 = w(-1, qv[c]), c0 = w(0, qv[c]), p1 = w(1, qv[c]), p2 = w(2, qv[c]);
-      dn[c] = (T(27) * (p1 - c0) - (p2 - m1)) * i24Xf;
-      fv[c] = (T(9) * (c0 + p1) - (m1 + p2)) * T(1.0 / 16.0);
-    }
-    T gt[4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-      gt[c] = (T(9) * (g(0, c) + g(1, c)) - (g(-1, c) + g(2, c))) * T(1.0 / 16.0);
-    T mu = viscosity<T>(gas, fv[3]);
-    T div = dn[0] + gt[1] + gt[3];
-    T tnn = mu * (T(2) * dn[0] - T(2.0 / 3.0) * div);
-    T tn1 = mu * (gt[0] + dn[1]);
-    T tn2 = mu * (gt[2] + dn[2]);
-    Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
-    Fr[4] -= fv[0] * tnn + fv[1] * tn1 + fv[2] * tn2 + mu * gas.lam_fac * dn[3];
-  }
-  F[0] = Fr[0]; F[1 + n] = Fr[1]; F[1 + t1] = Fr[2]; F[1 + t2] = Fr[3]; F[4] = Fr[4];
+  for (int c = 0; c < 5; ++c) F[rot_q<DIR>(c)] = Fr[c];
 }
 
 }  // namespace jf

@@ -67,7 +67,8 @@ def test_face_flux_matches_oracle_functions(jf, ora, d, kind):
     scale = np.maximum(np.max(np.abs(Fo), axis=1, keepdims=True), 1.0)
     assert np.max(np.abs(F - Fo) / scale) <= 5e-14
     F32 = jf.jf_diag_face_flux("f32", d, G, RG, PR, mu, W, Gt, Xf)
-    assert np.max(np.abs(F32 - Fo) / scale) <= 2e-5
+    # fp32 build of the same device code against the fp64 oracle: north_star's fp32 tolerance
+    assert np.max(np.abs(F32 - Fo) / scale) <= 1e-4
 
 
 def test_face_flux_consistency_on_uniform_stencils(jf, ora):
