@@ -157,10 +157,16 @@ struct RKArgs {
 // from lane l-1, evaluates the face pc-1/2 (HLLC + dissipative flux) and writes
 // R = -(F_{pc-1/2} - F_{pc-3/2})/dx for cell pc-1 (F_{pc-3/2} from lane l-1; lane 0: carried from
 // the previous iteration).  R is written, not accumulated: the x sweep runs first.
-constexpr int XS_WARPS = 8, XS_RING = 64;
+#ifndef JF_XS_WARPS
+#define JF_XS_WARPS 4
+#endif
+#ifndef JF_XS_MINB
+#define JF_XS_MINB 4
+#endif
+constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64;
 template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, bool VISC>
-__global__ void __launch_bounds__(XS_WARPS * 32)
+__global__ void __launch_bounds__(XS_WARPS * 32, JF_XS_MINB)
 sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* __restrict__ R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_y v, d_z u, d_z w]
@@ -281,16 +287,20 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     }
   };
   T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
-  // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots 0..4
-  for (int s = 0; s < YZ_RING; ++s) {
-    const long long o = col + (long long)(c0 + s) * sm;
+  // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots 0..4.
+  // All loads are issued before the first conversion so that their latencies overlap.
+  {
+    T raws[YZ_RING][5], gns[YZ_RING][4];
 #pragma unroll
-    for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + o];
-    if (VISC) {
+    for (int s = 0; s < YZ_RING; ++s) {
+      const long long o = col + (long long)(c0 + s) * sm;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) gn[c] = gsrc[c][(long long)(c0 + s) * sm];
+      for (int q = 0; q < 5; ++q) raws[s][q] = U[q * P.vol + o];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) gns[s][c] = VISC ? gsrc[c][(long long)(c0 + s) * sm] : T(0);
     }
-    put(s, raw, gn);
+#pragma unroll
+    for (int s = 0; s < YZ_RING; ++s) put(s, raws[s], gns[s]);
   }
   T WmPrev[5], Fprev[5];
 #pragma unroll
