@@ -65,7 +65,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+                                          "-lms", "25", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -133,6 +133,24 @@ def run_reference(args):
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------- multi-rank aggregation
+def max_over_ranks(times_ms, world, device=None):
+    """Replicas: every rank times its own box; the job's time is the slowest
+    rank's.  Returns the element-wise MAX over ranks of the local millisecond timings."""
+    if world <= 1:
+        return [float(t) for t in times_ms]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x) for x in times_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def job_throughput(cells_per_rank, steps, world, ms):
+    """Whole-job cell-updates/s: all ranks' cells x steps / the max-over-ranks time."""
+    return world * cells_per_rank * steps / (ms * 1e-3)
 
 
 # ---------------------------------------------------------------------------- our arm
@@ -210,16 +228,15 @@ def run_ours(args):
 
     # --- max over ranks
     if world > 1:
-        t = torch.tensor([ms, e2e[0] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t[0]); e2e = (float(t[1]), e2e[1]) if e2e else None
+        ms, e2e_ms = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, dev)
+        e2e = (e2e_ms, e2e[1]) if e2e else None
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     cells = case.cells
-    value = world * cells * K / (ms * 1e-3)
+    value = job_throughput(cells, K, world, ms)
     fm = flop_model(n)
     # roofline of the dominant kernel (bound: plain FP64/FP32 ALUs; nothing here is a contraction)
     peak_flops, _ = jf.jf_diag_alu_peak(args.dtype, 4096)
@@ -259,7 +276,7 @@ def run_ours(args):
         "kernels_ms_per_step": {k: v[0] / K for k, v in ktimes.items() if v[1]},
     }
     if e2e:
-        line["e2e"] = {"value": world * cells * e2e[1] / (e2e[0] * 1e-3), "unit": UNIT,
+        line["e2e"] = {"value": job_throughput(cells, e2e[1], world, e2e[0]), "unit": UNIT,
                        "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes, "ms_per_step": e2e[0] / e2e[1]}
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: one RK3 step of the SAME input on the host cores (the oracle as it stands)

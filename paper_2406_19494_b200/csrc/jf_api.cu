@@ -231,19 +231,19 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
 
 // Segment length of the marching (y / z) sweeps.  Each segment costs two extra WENO steps, one extra
 // face and a window prologue, so segments should be long; but the grid must still fill the 148 SMs
-// (3 resident 128-thread blocks each) for several waves.  Largest power-of-two length (<= N) that
-// leaves at least `waves` waves of blocks, never below 8 cells.
+// (12 resident warps each) for several waves.  Largest power-of-two length (<= N) that leaves at
+// least JF_SEG_WAVES waves of warps, never below 8 cells.
 #ifndef JF_SEG_WAVES
 #define JF_SEG_WAVES 4
 #endif
-int pick_segment(long long blocks_per_layer, int N) {
+int pick_segment(long long warps_per_layer, int N) {
 #ifdef JF_SEG_FORCE
   return JF_SEG_FORCE < N ? JF_SEG_FORCE : N;
 #endif
-  const long long want = (long long)JF_SEG_WAVES * 148 * 3;
+  const long long want = (long long)JF_SEG_WAVES * 148 * 12;
   int L = 8;
   while (L < N) L *= 2;                      // one segment
-  while (L > 8 && blocks_per_layer * ((N + L - 1) / L) < want) L /= 2;
+  while (L > 8 && warps_per_layer * ((N + L - 1) / L) < want) L /= 2;
   return L < N ? L : N;
 }
 
@@ -420,8 +420,8 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   const int n[3] = {g->nx, g->ny, g->nz};
   s->seg_len[0] = 0;
   auto cdiv = [](int a, int b) { return (long long)((a + b - 1) / b); };
-  s->seg_len[1] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[2], jf::YZ_TY), n[1]);
-  s->seg_len[2] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[1], jf::YZ_TY), n[2]);
+  s->seg_len[1] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[2], jf::YZ_TY) * jf::YZ_TY, n[1]);
+  s->seg_len[2] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[1], jf::YZ_TY) * jf::YZ_TY, n[2]);
   *out = s;
   return JF_OK;
 }

@@ -252,7 +252,10 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 #ifndef JF_YZ_MINB
 #define JF_YZ_MINB 3
 #endif
-constexpr int YZ_TX = 32, YZ_TY = 4, YZ_RING = 5;
+#ifndef JF_YZ_TY
+#define JF_YZ_TY 4
+#endif
+constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY, YZ_RING = 5;
 template <bool VISC> struct YZ { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, int DIR, bool VISC, int MODE>
 __global__ void __launch_bounds__(YZ_TX * YZ_TY, JF_YZ_MINB)

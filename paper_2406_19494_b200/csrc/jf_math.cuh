@@ -45,10 +45,20 @@ template <> struct Num<double> {
   static __device__ __forceinline__ double abs_(double a) { return fabs(a); }
 };
 template <> struct Num<float> {
-  static __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
   static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
-  static __device__ __forceinline__ float rcp(float a) { return 1.0f / a; }
-  static __device__ __forceinline__ float rsqrt_(float a) { return 1.0f / sqrtf(a); }
+  // MUFU seeds (rel. error ~2^-22) refined by one Newton step: ~1 ulp, a fraction of the IEEE sequences
+  static __device__ __forceinline__ float rcp(float a) {
+    float x;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(a));
+    return fmaf(x, fmaf(-a, x, 1.0f), x);
+  }
+  static __device__ __forceinline__ float rsqrt_(float a) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a));
+    float e = fmaf(-(a * y), y, 1.0f);
+    return fmaf(y, 0.5f * e, y);
+  }
+  static __device__ __forceinline__ float sqrt_(float a) { return a * rsqrt_(a); }
   static __device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
   static __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
   static __device__ __forceinline__ float abs_(float a) { return fabsf(a); }

@@ -267,6 +267,52 @@ def test_config4_tgv128_2_steps_fp64_and_fp32(jf, ora):
 
 
 # ------------------------------------------------------------------ error behaviour of the ABI
+# ------------------------------------------------------------------ full size, sampled (bench.py's launch configuration)
+def _sub_box_case(c, U, lo, m):
+    """Periodic m^3 case cut out of the periodic state U (full padded array) at interior offset lo."""
+    idx = [(np.arange(m) + lo[a]) % c.n[a] + NH for a in range(3)]
+    sub = cases.empty_state((m, m, m))
+    sub[(slice(None),) + (slice(NH, -NH),) * 3] = U[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+    dx = c.xf[1] - c.xf[0]
+    f = cases.uniform_faces(0.0, m * dx, m)
+    return cases.Case(name="sub", n=(m, m, m), xf=f, yf=f.copy(), zf=f.copy(), gamma=c.gamma, R_gas=c.R_gas,
+                      Pr=c.Pr, mu=c.mu, bc=cases.periodic_bc(), U0=sub, dt=c.dt, n_steps=1)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config4_tgv256_sampled_against_oracle_sub_boxes(jf, ora, dtype):
+    """256^3 (the size bench.py times, same kernels / grids / segment lengths): two RK3 steps on the GPU,
+    then the second step is checked on sampled 16^3 blocks.  One RK3 step moves information by at most
+    3 stages x 3 cells, so the oracle stepping a periodic 40^3 cut-out of the GPU's own step-1 state is
+    exact on the central 16^3 (margin 12 >= 9) whatever its (wrong) periodic wrap does at the rim."""
+    c = cases.tgv(256)
+    s = jf.Solver(c, dtype)
+    U = s.state()
+    s.jf_rk3_step(U, c.dt)
+    U1 = U.cpu().numpy().astype(np.float64)
+    s.jf_rk3_step(U, c.dt)
+    U2 = U.cpu().numpy().astype(np.float64)
+    m, g = 40, 12
+    rng = np.random.default_rng(11)
+    los = [(0, 0, 0), (250, 3, 121), (100, 250, 250)] + [tuple(int(v) for v in rng.integers(0, 256, 3)) for _ in range(3)]
+    mom = np.max(np.sqrt(U2[1] ** 2 + U2[2] ** 2 + U2[3] ** 2))
+    scale = [np.max(np.abs(U2[0])), mom, mom, mom, np.max(np.abs(U2[4]))]
+    worst = np.zeros(5)
+    for lo in los:
+        sc = _sub_box_case(c, U1, lo, m)
+        o = ora.Oracle(sc, dtype)
+        Uo = o.state()
+        o.rk3_step(Uo, c.dt)
+        Uo = np.asarray(Uo, dtype=np.float64)
+        idx = [(np.arange(g, m - g) + lo[a]) % 256 + NH for a in range(3)]
+        got = U2[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+        ref = Uo[:, NH + g:NH + m - g, NH + g:NH + m - g, NH + g:NH + m - g]
+        for q in range(5):
+            worst[q] = max(worst[q], np.max(np.abs(got[q] - ref[q])) / scale[q])
+    print("tgv256", dtype, "sampled parity", worst)
+    assert np.all(worst <= TOL[dtype]), worst
+
+
 def test_abi_error_statuses(jf):
     import ctypes as C
     import torch
