@@ -248,10 +248,16 @@ def run_ours(args):
     dom_ms, dom_n = ktimes[dom]
     dom_flops = alg.get(dom, 0.0) * cells
     achieved = dom_flops / (dom_ms / dom_n * 1e-3) / 1e12 if dom_n else 0.0
+    # measured DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of the
+    # committed ncu --set full capture; profiles/traffic.csv names its source), null if not captured for this size
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"{dom}|{n}|{args.dtype}")
+        import csv
+        with open(tpath) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == dom and int(row["size"]) == n and row["dtype"] == args.dtype:
+                    traffic = float(row["dram_bytes_per_launch"])
     peaks = {}
     ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(ppath):
