@@ -313,6 +313,45 @@ def test_config4_tgv256_sampled_against_oracle_sub_boxes(jf, ora, dtype):
     assert np.all(worst <= TOL[dtype]), worst
 
 
+# ------------------------------------------------------------------ out-of-bounds guard (compute-sanitizer is closed on this pool)
+@pytest.mark.parametrize("name", ["ragged", "tiny", "bc1"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_no_writes_outside_the_state_arrays(jf, name, dtype):
+    """U and R live inside larger buffers filled with a canary; after halo fill, RHS, CFL and an RK3 step
+    the guard bands (1 MiB on either side) must be untouched and every interior value finite."""
+    import torch
+    if name == "ragged":
+        c = cases.random_admissible(n=(70, 35, 67), seed=9, stretched=True)
+    elif name == "tiny":
+        c = cases.random_admissible(n=(4, 4, 4), seed=10)
+    else:
+        c = all_bc_case(n=(37, 21, 13), which=1)
+    s = jf.Solver(c, dtype)
+    n = int(np.prod(s.shape))
+    guard = (1 << 20) // (8 if dtype == "f64" else 4)
+    canary = -12345.678
+    bufs = [torch.full((n + 2 * guard,), canary, dtype=s.tdtype, device=s.device) for _ in range(2)]
+    U = bufs[0][guard:guard + n].view(s.shape)
+    U.copy_(s.state())
+    s.jf_fill_halo(U)
+    R = bufs[1][guard:guard + n].view(s.shape)
+    st = jf.lib().jf_rhs(s.h, s._ptr(U), s._ptr(R))
+    assert st == jf.JF_OK
+    st, dt = s.jf_cfl_dt(U, 0.4)
+    assert st == jf.JF_OK and dt > 0
+    s.jf_rk3_step(U, dt)
+    torch.cuda.synchronize()
+    for b in bufs:
+        assert bool((b[:guard] == canary).all()) and bool((b[guard + n:] == canary).all())
+    assert bool(torch.isfinite(U[(slice(None),) + (slice(NH, -NH),) * 3]).all())
+    Ri = R[(slice(None),) + (slice(NH, -NH),) * 3]
+    assert bool(torch.isfinite(Ri).all())
+    # jf_rhs leaves the halo cells of R untouched
+    mask = torch.ones(s.shape, dtype=torch.bool, device=s.device)
+    mask[(slice(None),) + (slice(NH, -NH),) * 3] = False
+    assert bool((R[mask] == canary).all())
+
+
 def test_abi_error_statuses(jf):
     import ctypes as C
     import torch
