@@ -42,7 +42,11 @@ typedef struct jf_solver jf_solver; /* opaque */
 typedef enum {
   JF_OK = 0, JF_EINVAL = 1, JF_EALIGN = 2, JF_EWORKSPACE = 3, JF_ECUDA = 4, JF_ENOTFINITE = 5
 } jf_status;
-typedef enum { JF_F64 = 0, JF_F32 = 1 } jf_dtype;
+/* JF_F64_TANGENT: forward-mode (tangent) solver.  Every state element is a pair of doubles
+ * (value, tangent), i.e. U_dev / R_dev hold jf_state_elems() pairs = 2*jf_state_elems() doubles,
+ * element e at doubles [2e] (value) and [2e+1] (directional derivative); the same kernels run on a
+ * dual-number scalar, so the value part follows the JF_F64 formulas.  See jf_set_tangent_seed. */
+typedef enum { JF_F64 = 0, JF_F32 = 1, JF_F64_TANGENT = 2 } jf_dtype;
 typedef enum {
   JF_BC_PERIODIC = 0, JF_BC_ZEROGRAD = 1, JF_BC_DIRICHLET = 2,
   JF_BC_WALL_ISOTHERMAL = 3, JF_BC_WALL_ADIABATIC = 4
@@ -114,6 +118,18 @@ jf_status jf_rk3_step(jf_solver *s, void *U_dev, double dt);
  * Writes *dt_host and synchronises the stream.  JF_ENOTFINITE (and *dt_host = NaN) if any
  * interior cell is non-finite or has rho <= 0 or p <= 0. */
 jf_status jf_cfl_dt(jf_solver *s, const void *U_dev, double cfl, double *dt_host);
+
+/* Tangent solvers (JF_F64_TANGENT) only; JF_EINVAL otherwise.  The paper introduces the Disturbance
+ * Wall so that its parameters can be differentiated through the solver.
+ * Sets the direction (dA, dkappa) in the parameter space of Eq. 8 (:112), applied to every disturbance
+ * segment: jf_fill_halo then seeds the wall-velocity tangent
+ *   d v_w = dA sin(2 pi kappa t1) + dkappa A 2 pi t1 cos(2 pi kappa t1),
+ * and jf_fill_halo / jf_rhs / jf_rk3_step propagate (value, tangent) pairs, so that after a step the
+ * tangent part of U is the directional derivative of the value part with respect to (A, kappa) along
+ * (dA, dkappa) (plus the propagated input tangent), at FIXED dt: jf_cfl_dt uses the value parts only
+ * and the tangent of dt is not propagated.  Non-smooth selections (min / max / sign in HLLC, the
+ * wall-temperature floor) take the derivative of the selected branch.  Default seed (0, 0). */
+jf_status jf_set_tangent_seed(jf_solver *s, double dA, double dkappa);
 
 /* Last error text of this solver ("" if none); never NULL. */
 const char *jf_last_error(const jf_solver *s);

@@ -13,7 +13,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libjf.so")
 
 JF_OK, JF_EINVAL, JF_EALIGN, JF_EWORKSPACE, JF_ECUDA, JF_ENOTFINITE = range(6)
-JF_F64, JF_F32 = 0, 1
+JF_F64, JF_F32, JF_F64_TANGENT = 0, 1, 2
+_DTYPES = {"f64": JF_F64, "f32": JF_F32, "f64t": JF_F64_TANGENT}
 _STATUS = {0: "JF_OK", 1: "JF_EINVAL", 2: "JF_EALIGN", 3: "JF_EWORKSPACE", 4: "JF_ECUDA", 5: "JF_ENOTFINITE"}
 
 c_double_p = C.POINTER(C.c_double)
@@ -43,7 +44,7 @@ class jf_bc(C.Structure):
 
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
-           "jf_rk3_step", "jf_cfl_dt", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
+           "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_version"]
 
 _lib = None
@@ -76,6 +77,8 @@ def lib():
         L.jf_fill_halo.argtypes = [C.c_void_p, C.c_void_p]
         L.jf_rhs.restype = C.c_int
         L.jf_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.jf_set_tangent_seed.restype = C.c_int
+        L.jf_set_tangent_seed.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.jf_rk3_step.restype = C.c_int
         L.jf_rk3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
         L.jf_cfl_dt.restype = C.c_int
@@ -144,7 +147,8 @@ class Solver:
     """jf_solver handle + its device workspace, built from a cases.Case description.
 
     Methods carry the names of the C calls; tensors are torch CUDA tensors of the solver dtype
-    and shape [5, nz+6, ny+6, nx+6]."""
+    and shape [5, nz+6, ny+6, nx+6]; dtype "f64t" (JF_F64_TANGENT) adds a trailing axis of 2:
+    [..., 0] value, [..., 1] tangent."""
 
     def __init__(self, case, dtype="f64", device="cuda:0", stream=None):
         import torch
@@ -154,11 +158,11 @@ class Solver:
         self.case = case
         self.device = torch.device(device)
         self.dtype = dtype
-        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self.tdtype = torch.float32 if dtype == "f32" else torch.float64
         self._keep = []
         L = lib()
         g = _grid_struct(case, self._keep)
-        dt = JF_F64 if dtype == "f64" else JF_F32
+        dt = _DTYPES[dtype]
         nbytes = L.jf_workspace_bytes(C.byref(g), dt)
         if nbytes == 0:
             raise JFError(JF_EINVAL, "jf_workspace_bytes")
@@ -195,6 +199,8 @@ class Solver:
         nx, ny, nz = case.n
         self.shape = (5, nz + 6, ny + 6, nx + 6)
         assert L.jf_state_elems(h) == int(np.prod(self.shape))
+        if dtype == "f64t":
+            self.shape = self.shape + (2,)
 
     def close(self):
         if getattr(self, "h", None):
@@ -215,10 +221,17 @@ class Solver:
         assert t.is_cuda and t.dtype == self.tdtype and t.is_contiguous() and tuple(t.shape) == self.shape
         return C.c_void_p(t.data_ptr())
 
-    def state(self, U0=None):
-        """Device copy of a host state array (case.U0 by default)."""
+    def state(self, U0=None, dU0=None):
+        """Device copy of a host state array (case.U0 by default); tangent solvers interleave
+        (value, tangent) with the tangent dU0 (zero by default)."""
         U = np.asarray(self.case.U0 if U0 is None else U0)
+        if self.dtype == "f64t":
+            dU = np.zeros_like(U) if dU0 is None else np.asarray(dU0)
+            U = np.stack([U, dU], axis=-1)
         return self.torch.as_tensor(U, dtype=self.tdtype).contiguous().to(self.device)
+
+    def jf_set_tangent_seed(self, dA, dkappa):
+        self._check(lib().jf_set_tangent_seed(self.h, float(dA), float(dkappa)))
 
     def jf_fill_halo(self, U):
         self._check(lib().jf_fill_halo(self.h, self._ptr(U)))

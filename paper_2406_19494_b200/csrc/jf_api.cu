@@ -88,12 +88,16 @@ struct Impl {
   unsigned long long* cfl_out;
 };
 
+bool dtype_ok(jf_dtype d) { return d == JF_F64 || d == JF_F32 || d == JF_F64_TANGENT; }
+size_t elem_size(jf_dtype d) { return d == JF_F64 ? sizeof(double) : (d == JF_F32 ? sizeof(float) : sizeof(jf::Dual)); }
+
 }  // namespace
 
 struct jf_solver {
   jf_dtype dtype;
   Impl<double> d;
   Impl<float> f;
+  Impl<jf::Dual> t;              // JF_F64_TANGENT: (value, tangent) pairs
   cudaStream_t stream;
   bool viscous;
   double Pr;
@@ -216,6 +220,7 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
     const bool wall = b.type == JF_BC_WALL_ISOTHERMAL || b.type == JF_BC_WALL_ADIABATIC;
     o.dist_on = wall && b.dist.enabled;
     o.A = b.dist.A; o.kappa = b.dist.kappa; o.lo = b.dist.t1_lo; o.hi = b.dist.t1_hi;
+    o.dA = 0.0; o.dkappa = 0.0;
     o.dirichlet = nullptr;
     if (b.type == JF_BC_DIRICHLET) {
       int a = f / 2, t1 = (a == 0) ? 1 : 0, t2 = (a == 2) ? 1 : 2;
@@ -374,9 +379,9 @@ jf_status cfl(jf_solver* s, Impl<T>& I, const T* U, double cflnum, double* dt_ho
 extern "C" {
 
 size_t jf_workspace_bytes(const jf_grid* g, jf_dtype dtype) {
-  if (!grid_ok(g) || (dtype != JF_F64 && dtype != JF_F32)) return 0;
+  if (!grid_ok(g) || !dtype_ok(dtype)) return 0;
   const int n[3] = {g->nx, g->ny, g->nz};
-  return make_layout(n, dtype == JF_F64 ? sizeof(double) : sizeof(float)).total;
+  return make_layout(n, elem_size(dtype)).total;
 }
 
 jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double gamma, double R_gas, double Pr,
@@ -385,7 +390,7 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   if (!out) return JF_EINVAL;
   *out = nullptr;
   if (!grid_ok(g) || !mu || !bc) return JF_EINVAL;
-  if (dtype != JF_F64 && dtype != JF_F32) return JF_EINVAL;
+  if (!dtype_ok(dtype)) return JF_EINVAL;
   if (!(gamma > 1.0) || !(R_gas > 0.0) || !(Pr > 0.0) || !(mu->mu_ref >= 0.0)) return JF_EINVAL;
   if (mu->sutherland && !(mu->T_ref > 0.0)) return JF_EINVAL;
   for (int a = 0; a < 3; ++a)
@@ -408,13 +413,14 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   s->viscous = mu->mu_ref > 0.0;
   s->Pr = Pr;
   s->launches = 0;
-  jf_status st = dtype == JF_F64
-                     ? setup<double>(s, s->d, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev)
-                     : setup<float>(s, s->f, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev);
+  jf_status st = dtype == JF_F64   ? setup<double>(s, s->d, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev)
+                 : dtype == JF_F32 ? setup<float>(s, s->f, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev)
+                                   : setup<jf::Dual>(s, s->t, g, gamma, R_gas, Pr, mu, bc, body_accel, (char*)workspace_dev);
   if (st != JF_OK) { delete s; return st; }
   {
-    cudaError_t ce = dtype == JF_F64 ? (s->viscous ? opt_in_smem<double, true>() : opt_in_smem<double, false>())
-                                     : (s->viscous ? opt_in_smem<float, true>() : opt_in_smem<float, false>());
+    cudaError_t ce = dtype == JF_F64   ? (s->viscous ? opt_in_smem<double, true>() : opt_in_smem<double, false>())
+                     : dtype == JF_F32 ? (s->viscous ? opt_in_smem<float, true>() : opt_in_smem<float, false>())
+                                       : (s->viscous ? opt_in_smem<jf::Dual, true>() : opt_in_smem<jf::Dual, false>());
     if (ce != cudaSuccess) { delete s; return JF_ECUDA; }
   }
   const int n[3] = {g->nx, g->ny, g->nz};
@@ -463,7 +469,7 @@ const char* jf_diag_kernel_name(int k) {
 
 size_t jf_state_elems(const jf_solver* s) {
   if (!s) return 0;
-  return s->dtype == JF_F64 ? (size_t)5 * s->d.P.vol : (size_t)5 * s->f.P.vol;
+  return (size_t)5 * (s->dtype == JF_F64 ? s->d.P.vol : s->dtype == JF_F32 ? s->f.P.vol : s->t.P.vol);
 }
 
 static bool aligned16(const void* p) { return ((uintptr_t)p) % 16 == 0; }
@@ -472,30 +478,44 @@ jf_status jf_fill_halo(jf_solver* s, void* U) {
   if (!s) return JF_EINVAL;
   if (!U) return fail(s, JF_EINVAL, "jf_fill_halo: null pointer");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_fill_halo: U not 16-byte aligned");
-  return s->dtype == JF_F64 ? launch_halo<double>(s, s->d, (double*)U) : launch_halo<float>(s, s->f, (float*)U);
+  return s->dtype == JF_F64   ? launch_halo<double>(s, s->d, (double*)U)
+         : s->dtype == JF_F32 ? launch_halo<float>(s, s->f, (float*)U)
+                              : launch_halo<jf::Dual>(s, s->t, (jf::Dual*)U);
 }
 
 jf_status jf_rhs(jf_solver* s, const void* U, void* R) {
   if (!s) return JF_EINVAL;
   if (!U || !R || U == R) return fail(s, JF_EINVAL, "jf_rhs: null or aliased pointers");
   if (!aligned16(U) || !aligned16(R)) return fail(s, JF_EALIGN, "jf_rhs: pointer not 16-byte aligned");
-  return s->dtype == JF_F64 ? launch_rhs<double>(s, s->d, (const double*)U, (double*)R, nullptr)
-                            : launch_rhs<float>(s, s->f, (const float*)U, (float*)R, nullptr);
+  return s->dtype == JF_F64   ? launch_rhs<double>(s, s->d, (const double*)U, (double*)R, nullptr)
+         : s->dtype == JF_F32 ? launch_rhs<float>(s, s->f, (const float*)U, (float*)R, nullptr)
+                              : launch_rhs<jf::Dual>(s, s->t, (const jf::Dual*)U, (jf::Dual*)R, nullptr);
 }
 
 jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
   if (!s) return JF_EINVAL;
   if (!U || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_step: null pointer or NaN dt");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_step: U not 16-byte aligned");
-  return s->dtype == JF_F64 ? rk3<double>(s, s->d, (double*)U, dt) : rk3<float>(s, s->f, (float*)U, dt);
+  return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, dt)
+         : s->dtype == JF_F32 ? rk3<float>(s, s->f, (float*)U, dt)
+                              : rk3<jf::Dual>(s, s->t, (jf::Dual*)U, dt);
 }
 
 jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host) {
   if (!s) return JF_EINVAL;
   if (!U || !dt_host) return fail(s, JF_EINVAL, "jf_cfl_dt: null pointer");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_cfl_dt: U not 16-byte aligned");
-  return s->dtype == JF_F64 ? cfl<double>(s, s->d, (const double*)U, cflnum, dt_host)
-                            : cfl<float>(s, s->f, (const float*)U, cflnum, dt_host);
+  return s->dtype == JF_F64   ? cfl<double>(s, s->d, (const double*)U, cflnum, dt_host)
+         : s->dtype == JF_F32 ? cfl<float>(s, s->f, (const float*)U, cflnum, dt_host)
+                              : cfl<jf::Dual>(s, s->t, (const jf::Dual*)U, cflnum, dt_host);
+}
+
+jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {
+  if (!s) return JF_EINVAL;
+  if (s->dtype != JF_F64_TANGENT) return fail(s, JF_EINVAL, "jf_set_tangent_seed: not a tangent solver");
+  if (!(dA == dA) || !(dkappa == dkappa)) return fail(s, JF_EINVAL, "jf_set_tangent_seed: NaN seed");
+  for (int f = 0; f < 6; ++f) { s->t.bc[f].dA = dA; s->t.bc[f].dkappa = dkappa; }
+  return JF_OK;
 }
 
 const char* jf_last_error(const jf_solver* s) { return s ? s->err.c_str() : ""; }

@@ -37,6 +37,7 @@ struct FaceBC {
   T T_wall, uw[3];
   int dist_on;
   double A, kappa, lo, hi;
+  double dA, dkappa;            // tangent direction in (A, kappa) (tangent solvers; else 0)
   const double* dirichlet;      // device, prim[5][n_t2][n_t1]
 };
 
@@ -91,8 +92,11 @@ __global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, F
       double t1 = P.xc[t1a][p1];
       if (t1 >= f.lo && t1 <= f.hi) {
         // Eq. 8: v_w = A sin(2 pi kappa t1), wall-normal component
-        double vw = f.A * sin(2.0 * 3.14159265358979323846 * f.kappa * t1);
-        uw[AXIS] = uw[AXIS] + T(vw);
+        const double ph = 2.0 * 3.14159265358979323846 * f.kappa * t1, sn = sin(ph);
+        const double vw = f.A * sn;
+        // directional derivative of v_w along (dA, dkappa): used by the tangent instantiation only
+        const double dvw = f.dA * sn + f.dkappa * f.A * (2.0 * 3.14159265358979323846 * t1) * cos(ph);
+        uw[AXIS] = uw[AXIS] + with_tangent<T>(vw, dvw);
       }
     }
     W[1] = T(2) * uw[0] - Wr[1]; W[2] = T(2) * uw[1] - Wr[2]; W[3] = T(2) * uw[2] - Wr[3];
@@ -223,7 +227,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     T WL[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      WL[q] = __shfl_sync(full, lane == 31 ? WmOld[q] : Wm[q], src_lane);
+      WL[q] = shfl(full, lane == 31 ? WmOld[q] : Wm[q], src_lane);
       WmOld[q] = Wm[q];
     }
     T F[5] = {T(0), T(0), T(0), T(0), T(0)};
@@ -232,7 +236,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     const T idl = (pc >= 4 && pc <= nx + 3) ? P.inv_dl[0][pc - 1] : T(0);
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      T Fm = __shfl_sync(full, lane == 31 ? Fold[q] : F[q], src_lane);
+      T Fm = shfl(full, lane == 31 ? Fold[q] : F[q], src_lane);
       Fold[q] = F[q];
       if (pc >= 4 && pc <= nx + 3) R[q * P.vol + base + pc - 1] = -(F[q] - Fm) * idl;
     }
@@ -389,7 +393,7 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
     T r = U[o], mx = U[P.vol + o], my = U[2 * P.vol + o], mz = U[3 * P.vol + o], E = U[4 * P.vol + o];
     T u = mx / r, v = my / r, w = mz / r;
     T p = gas.gm1 * (E - T(0.5) * r * (u * u + v * v + w * w));
-    bool ok = isfinite(r) && isfinite(mx) && isfinite(my) && isfinite(mz) && isfinite(E) && (r > T(0)) && (p > T(0));
+    bool ok = finite_(r) && finite_(mx) && finite_(my) && finite_(mz) && finite_(E) && (r > T(0)) && (p > T(0));
     if (!ok) { bad = 1; continue; }
     T cs = Num<T>::sqrt_(gas.gamma * p / r);
     T dl[3] = {P.dl[0][i + NH], P.dl[1][j + NH], P.dl[2][k + NH]};
@@ -410,9 +414,9 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
   }
 #pragma unroll
   for (int s = 16; s > 0; s >>= 1) {
-    dconv = Num<T>::min_(dconv, __shfl_xor_sync(0xffffffffu, dconv, s));
-    dvisc = Num<T>::min_(dvisc, __shfl_xor_sync(0xffffffffu, dvisc, s));
-    dheat = Num<T>::min_(dheat, __shfl_xor_sync(0xffffffffu, dheat, s));
+    dconv = Num<T>::min_(dconv, shfl_xor(0xffffffffu, dconv, s));
+    dvisc = Num<T>::min_(dvisc, shfl_xor(0xffffffffu, dvisc, s));
+    dheat = Num<T>::min_(dheat, shfl_xor(0xffffffffu, dheat, s));
     bad |= __shfl_xor_sync(0xffffffffu, bad, s);
   }
   __shared__ double sred[3][8];

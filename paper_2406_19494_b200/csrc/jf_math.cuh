@@ -16,6 +16,7 @@
 // Results agree with the closed forms to a few ulp, not bit-wise (tolerance: DESIGN.md).
 #pragma once
 #include <cuda_runtime.h>
+#include "jf_dual.cuh"
 
 namespace jf {
 
@@ -63,6 +64,40 @@ template <> struct Num<float> {
   static __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
   static __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
 };
+
+// tangent scalar: value part by the same formulas as Num<double>, tangent by the chain rule
+template <> struct Num<Dual> {
+  using D = Num<double>;
+  static __device__ __forceinline__ Dual fma_(Dual a, Dual b, Dual c) {
+    return Dual(fma(a.v, b.v, c.v), fma(a.v, b.d, fma(a.d, b.v, c.d)));
+  }
+  static __device__ __forceinline__ Dual rcp(Dual a) { const double r = D::rcp(a.v); return Dual(r, -a.d * r * r); }
+  static __device__ __forceinline__ Dual rsqrt_(Dual a) {
+    const double y = D::rsqrt_(a.v);
+    return Dual(y, -0.5 * a.d * y * y * y);
+  }
+  static __device__ __forceinline__ Dual sqrt_(Dual a) {
+    const double y = D::rsqrt_(a.v);
+    return Dual(a.v * y, 0.5 * a.d * y);
+  }
+  static __device__ __forceinline__ Dual min_(Dual a, Dual b) { return b.v < a.v ? b : a; }
+  static __device__ __forceinline__ Dual max_(Dual a, Dual b) { return b.v > a.v ? b : a; }
+  static __device__ __forceinline__ Dual abs_(Dual a) { return a.v < 0.0 ? -a : a; }
+};
+
+// warp shuffles / finiteness / (value, tangent) construction, generic over the scalar type
+template <class T> __device__ __forceinline__ T shfl(unsigned m, T a, int src) { return __shfl_sync(m, a, src); }
+__device__ __forceinline__ Dual shfl(unsigned m, Dual a, int src) {
+  return Dual(__shfl_sync(m, a.v, src), __shfl_sync(m, a.d, src));
+}
+template <class T> __device__ __forceinline__ T shfl_xor(unsigned m, T a, int lm) { return __shfl_xor_sync(m, a, lm); }
+__device__ __forceinline__ Dual shfl_xor(unsigned m, Dual a, int lm) {
+  return Dual(__shfl_xor_sync(m, a.v, lm), __shfl_xor_sync(m, a.d, lm));
+}
+template <class T> __device__ __forceinline__ bool finite_(T a) { return isfinite(a); }
+__device__ __forceinline__ bool finite_(Dual a) { return isfinite(a.v) && isfinite(a.d); }
+template <class T> __device__ __forceinline__ T with_tangent(double v, double) { return T(v); }
+template <> __device__ __forceinline__ Dual with_tangent<Dual>(double v, double d) { return Dual(v, d); }
 
 // gas / transport constants handed to every kernel
 template <class T>
