@@ -155,19 +155,26 @@ struct RKArgs {
 };
 
 // ------------------------------------------------------------------ x sweep
-// One warp per (j,k) line.  Iteration kc loads padded cells [32kc, 32kc+32) (prefetched one
-// iteration ahead), converts them to primitives in a 64-cell warp-private ring, then lane l does
-// the per-cell WENO of padded cell pc = 32kc-2+l (W^-_{pc+1/2}, W^+_{pc-1/2}), takes W^-_{pc-1/2}
-// from lane l-1, evaluates the face pc-1/2 (HLLC + dissipative flux) and writes
-// R = -(F_{pc-1/2} - F_{pc-3/2})/dx for cell pc-1 (F_{pc-3/2} from lane l-1; lane 0: carried from
-// the previous iteration).  R is written, not accumulated: the x sweep runs first.
+// One warp per group of XS_LINES consecutive (j,k) lines, treated as ONE stream of padded cells
+// (line after line), so that the 32-cell iterations stay full across line ends (a 256-cell line
+// needs 258 cells = 8.06 iterations: 9 when lines are swept one by one).  Iteration kc loads the
+// stream cells [32kc, 32kc+32) (prefetched one iteration ahead), converts them to primitives in a
+// 64-cell warp-private ring, then lane l does the per-cell WENO of stream cell 32kc-2+l = padded
+// cell pc of its line (W^-_{pc+1/2}, W^+_{pc-1/2}), takes W^-_{pc-1/2} from lane l-1, evaluates the
+// face pc-1/2 (HLLC + dissipative flux) and writes R = -(F_{pc-1/2} - F_{pc-3/2})/dx for cell pc-1
+// (F_{pc-3/2} from lane l-1; lane 0: carried from the previous iteration).  A WENO cell (2 <= pc <=
+// nx+3) and the cell the same lane loaded (pc+2) lie on the same line, so one (line base, p) pair per
+// lane serves both; windows never cross a line end.  R is written, not accumulated: x runs first.
 #ifndef JF_XS_WARPS
 #define JF_XS_WARPS 4
 #endif
 #ifndef JF_XS_MINB
 #define JF_XS_MINB 4
 #endif
-constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64;
+#ifndef JF_XS_LINES
+#define JF_XS_LINES 4
+#endif
+constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES;
 template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, bool VISC>
 __global__ void __launch_bounds__(XS_WARPS * 32, JF_XS_MINB)
@@ -175,37 +182,51 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_y v, d_z u, d_z w]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int row = blockIdx.x * XS_WARPS + warp;
   const int ny = P.n[1], nz = P.n[2], nx = P.n[0], Px = P.P[0];
-  if (row >= ny * nz) return;
-  const int j = row % ny, k = row / ny;
-  const long long base = (long long)(k + NH) * P.sz + (long long)(j + NH) * P.sy;
+  const int rows = ny * nz;
+  const int row0 = (blockIdx.x * XS_WARPS + warp) * XS_LINES;
+  if (row0 >= rows) return;
+  const int S = min(XS_LINES, rows - row0) * Px;            // stream length of this warp
   T* ring = reinterpret_cast<T*>(smem_raw) + warp * (NV * XS_RING);
   const Gas<T> gas = P.gas;
-  const T* gsrc[4] = {G + (long long)(3 * 1 + 0) * P.vol + base, G + (long long)(3 * 1 + 1) * P.vol + base,
-                      G + (long long)(3 * 2 + 0) * P.vol + base, G + (long long)(3 * 2 + 2) * P.vol + base};
-  const int kmax = (nx + 5) / 32;            // last cell to treat: pc = nx+3
+  const long long gv[4] = {(long long)(3 * 1 + 0) * P.vol, (long long)(3 * 1 + 1) * P.vol,   // d_y u, d_y v
+                           (long long)(3 * 2 + 0) * P.vol, (long long)(3 * 2 + 2) * P.vol};  // d_z u, d_z w
+  const int kmax = (S - 1) / 32;             // last stream cell to treat: S-3 (pc = nx+3 of the last line)
   const unsigned full = 0xffffffffu;
   const int src_lane = (lane + 31) & 31;
-  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
-  auto fetch = [&](int p) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) raw[q] = (p < Px) ? U[q * P.vol + base + p] : T(1);
-    if (VISC) {
-#pragma unroll
-      for (int c = 0; c < 4; ++c) gn[c] = (p < Px) ? gsrc[c][p] : T(0);
+  // this lane's load cell: stream index 32kc+lane = padded cell p of line (j,k), advanced by 32 per iteration
+  int p, j, k;
+  {
+    const int l = lane / Px, row = row0 + l;
+    p = lane - l * Px; j = row % ny; k = row / ny;
+  }
+  long long base = (long long)(k + NH) * P.sz + (long long)(j + NH) * P.sy;
+  auto advance = [&]() {                     // to the cell loaded in the next iteration
+    p += 32;
+    while (p >= Px) {
+      p -= Px;
+      if (++j == ny) { j = 0; ++k; base += P.sz - (long long)(ny - 1) * P.sy; } else base += P.sy;
     }
   };
-  fetch(lane);
+  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
+  auto fetch = [&](bool in) {                // the cell at (base, p); `in`: inside this warp's stream
+#pragma unroll
+    for (int q = 0; q < 5; ++q) raw[q] = in ? U[q * P.vol + base + p] : T(1);
+    if (VISC) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) gn[c] = in ? G[gv[c] + base + p] : T(0);
+    }
+  };
+  fetch(lane < S);
   T WmOld[5], Fold[5];                       // this lane's W^- and F of the previous iteration
 #pragma unroll
   for (int q = 0; q < 5; ++q) { WmOld[q] = T(1); Fold[q] = T(0); }
   for (int kc = 0; kc <= kmax; ++kc) {
-    const int p = 32 * kc + lane;
-    if (p < Px) {
+    const int t = 32 * kc + lane;            // stream index of the loaded cell
+    if (t < S) {
       T W[6];
       cons_to_prim<T>(gas, raw[0], raw[1], raw[2], raw[3], raw[4], W);
-      T* dst = ring + (p & (XS_RING - 1));
+      T* dst = ring + (t & (XS_RING - 1));
 #pragma unroll
       for (int q = 0; q < 5; ++q) dst[q * XS_RING] = W[q];
       if (VISC) {
@@ -214,15 +235,19 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
         for (int c = 0; c < 4; ++c) dst[(6 + c) * XS_RING] = gn[c];
       }
     }
-    if (kc < kmax) fetch(p + 32);
+    // WENO cell of this lane: stream index t-2 = padded cell pc = p-2 of the same line (if p >= 4)
+    const int pc = p - 2;
+    const long long cbase = base;
+    const bool cell = t < S && p >= 4;       // 2 <= pc <= nx+3
+    if (kc < kmax) { advance(); fetch(t + 32 < S); }
     __syncwarp();
-    const int pc = 32 * kc - 2 + lane;
-    auto w = [&](int m, int q) -> T { return ring[q * XS_RING + ((pc + m) & (XS_RING - 1))]; };
-    auto g = [&](int m, int c) -> T { return ring[(6 + c) * XS_RING + ((pc + m) & (XS_RING - 1))]; };
+    const int tc = t - 2;
+    auto w = [&](int m, int q) -> T { return ring[q * XS_RING + ((tc + m) & (XS_RING - 1))]; };
+    auto g = [&](int m, int c) -> T { return ring[(6 + c) * XS_RING + ((tc + m) & (XS_RING - 1))]; };
     T Wm[5], Wp[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) { Wm[q] = T(1); Wp[q] = T(1); }
-    if (pc >= 2 && pc <= nx + 3) weno_cell_states<T, 0>(w, Wm, Wp);
+    if (cell) weno_cell_states<T, 0>(w, Wm, Wp);
     // W^-_{pc-1/2} comes from lane-1; lane 0 takes lane 31's value of the previous iteration
     T WL[5];
 #pragma unroll
@@ -231,14 +256,15 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
       WmOld[q] = Wm[q];
     }
     T F[5] = {T(0), T(0), T(0), T(0), T(0)};
-    if (pc >= 3 && pc <= nx + 3)
+    if (cell && pc >= 3)
       face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][pc - 1] : T(0), F);
-    const T idl = (pc >= 4 && pc <= nx + 3) ? P.inv_dl[0][pc - 1] : T(0);
+    const bool upd = cell && pc >= 4;
+    const T idl = upd ? P.inv_dl[0][pc - 1] : T(0);
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       T Fm = shfl(full, lane == 31 ? Fold[q] : F[q], src_lane);
       Fold[q] = F[q];
-      if (pc >= 4 && pc <= nx + 3) R[q * P.vol + base + pc - 1] = -(F[q] - Fm) * idl;
+      if (upd) R[q * P.vol + cbase + pc - 1] = -(F[q] - Fm) * idl;
     }
     __syncwarp();
   }
