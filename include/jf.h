@@ -47,9 +47,13 @@ typedef enum {
  * element e at doubles [2e] (value) and [2e+1] (directional derivative); the same kernels run on a
  * dual-number scalar, so the value part follows the JF_F64 formulas.  See jf_set_tangent_seed. */
 typedef enum { JF_F64 = 0, JF_F32 = 1, JF_F64_TANGENT = 2 } jf_dtype;
+/* JF_BC_EXCHANGE: the face adjoins another block of a block-decomposed domain (equal
+ * blocks, one per device, halo exchange with exactly one neighbour per face).  jf_fill_halo leaves its
+ * halo layers alone; the caller fills them from the neighbour with jf_pull_face or jf_pack_face /
+ * jf_unpack_face, axis by axis (see "Block decomposition" below). */
 typedef enum {
   JF_BC_PERIODIC = 0, JF_BC_ZEROGRAD = 1, JF_BC_DIRICHLET = 2,
-  JF_BC_WALL_ISOTHERMAL = 3, JF_BC_WALL_ADIABATIC = 4
+  JF_BC_WALL_ISOTHERMAL = 3, JF_BC_WALL_ADIABATIC = 4, JF_BC_EXCHANGE = 5
 } jf_bc_type;
 
 /* Grid: face coordinates per axis (host pointers, copied by jf_create), strictly increasing.
@@ -78,6 +82,9 @@ typedef struct {
                               (rho,u,v,w,p) over the interior tangential sizes (x faces:
                               t1=y,t2=z; y faces: t1=x,t2=z; z faces: t1=x,t2=y); copied     */
   jf_disturbance dist;     /* walls only */
+  double nb_width[3];      /* JF_BC_EXCHANGE: widths of the neighbouring block's three cells next to
+                              this face, nearest first (> 0): the halo cells then carry the geometry
+                              they have on the undivided grid (stretched axes included)              */
 } jf_bc_face;
 typedef struct { jf_bc_face face[6]; } jf_bc; /* x-, x+, y-, y+, z-, z+; periodic must pair */
 
@@ -118,6 +125,46 @@ jf_status jf_rk3_step(jf_solver *s, void *U_dev, double dt);
  * Writes *dt_host and synchronises the stream.  JF_ENOTFINITE (and *dt_host = NaN) if any
  * interior cell is non-finite or has rho <= 0 or p <= 0. */
 jf_status jf_cfl_dt(jf_solver *s, const void *U_dev, double cfl, double *dt_host);
+
+/* ---- Block decomposition ------------------------------------------
+ * One solver per block; faces between blocks are JF_BC_EXCHANGE.  One RK stage of a decomposed step is
+ *   for axis in x, y, z:   every block: jf_fill_halo_axis(axis)            (its physical faces)
+ *                          every block: for its exchange faces of that axis: jf_pull_face from the
+ *                                       neighbour's stage input (or pack -> transport -> unpack)
+ *   every block: jf_rk3_stage_advance(stage)
+ * with the stage inputs given by jf_rk3_stage_input.  The axis order and the tangential extents of each
+ * pass (x: interior (j,k); y: all padded i, interior k; z: all padded (i,j)) are those of jf_fill_halo, so
+ * edges and corners come out exactly as on the undivided grid: a decomposed run reproduces the undivided
+ * one cell for cell.  All calls are asynchronous on the solver's stream; ordering BETWEEN blocks (the
+ * neighbour must have finished the previous axis pass, and must not overwrite the array before it was
+ * read) is the caller's: same stream, events, or a barrier between ranks. */
+
+/* Boundary pass of one axis (0 x, 1 y, 2 z) only; jf_fill_halo = axes 0, 1, 2 in this order. */
+jf_status jf_fill_halo_axis(jf_solver *s, void *U_dev, int axis);
+
+/* Elements (of the solver dtype; pairs for tangent solvers) of one packed face buffer:
+ * 5 * 3 * (tangential cells of that axis' pass); 0 on bad arguments. */
+size_t jf_face_elems(const jf_solver *s, int face);
+
+/* Pack the three interior layers next to `face` (0..5 = x-, x+, y-, y+, z-, z+) into buf_dev
+ * [5][3][n_t2][n_t1] - what the neighbour across that face needs for ITS opposite face; unpack writes
+ * such a buffer (packed by the neighbour across `face` for its opposite face) into the halo layers of
+ * `face`.  Layer m = 1..3 counts outward from the face on both sides. */
+jf_status jf_pack_face(jf_solver *s, const void *U_dev, int face, void *buf_dev);
+jf_status jf_unpack_face(jf_solver *s, void *U_dev, int face, const void *buf_dev);
+
+/* Fill the halo layers of `face` directly from the neighbouring block's state array U_peer_dev (same
+ * layout and dtype; a pointer on this device or a peer-mapped one: the loads then cross NVLink inside
+ * the kernel, no staging buffer).  n_peer = the peer block's interior sizes: equal to this block's in the
+ * two tangential axes (else JF_EINVAL). */
+jf_status jf_pull_face(jf_solver *s, void *U_dev, int face, const void *U_peer_dev, const int n_peer[3]);
+
+/* The array whose halos stage 1, 2, 3 of jf_rk3_step reads: U_dev itself (stage 1) or one of the
+ * solver's two stage buffers inside the workspace; NULL on bad arguments.  jf_rk3_stage_advance runs
+ * R_NSE and the SSP-RK3 update of that stage, assuming the halos of its input are filled:
+ * jf_rk3_step(U, dt) == for stage 1..3: jf_fill_halo(jf_rk3_stage_input(U, stage)); advance(U, stage, dt). */
+void *jf_rk3_stage_input(jf_solver *s, void *U_dev, int stage);
+jf_status jf_rk3_stage_advance(jf_solver *s, void *U_dev, int stage, double dt);
 
 /* Tangent solvers (JF_F64_TANGENT) only; JF_EINVAL otherwise.  The paper introduces the Disturbance
  * Wall so that its parameters can be differentiated through the solver.

@@ -36,7 +36,7 @@ class jf_disturbance(C.Structure):
 
 class jf_bc_face(C.Structure):
     _fields_ = [("type", C.c_int), ("T_wall", C.c_double), ("u_wall", C.c_double * 3),
-                ("dirichlet", c_double_p), ("dist", jf_disturbance)]
+                ("dirichlet", c_double_p), ("dist", jf_disturbance), ("nb_width", C.c_double * 3)]
 
 
 class jf_bc(C.Structure):
@@ -44,7 +44,8 @@ class jf_bc(C.Structure):
 
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
-           "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
+           "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
+           "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_version"]
 
 _lib = None
@@ -77,6 +78,20 @@ def lib():
         L.jf_fill_halo.argtypes = [C.c_void_p, C.c_void_p]
         L.jf_rhs.restype = C.c_int
         L.jf_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.jf_fill_halo_axis.restype = C.c_int
+        L.jf_fill_halo_axis.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.jf_face_elems.restype = C.c_size_t
+        L.jf_face_elems.argtypes = [C.c_void_p, C.c_int]
+        L.jf_pack_face.restype = C.c_int
+        L.jf_pack_face.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.jf_unpack_face.restype = C.c_int
+        L.jf_unpack_face.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.jf_pull_face.restype = C.c_int
+        L.jf_pull_face.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_int)]
+        L.jf_rk3_stage_input.restype = C.c_void_p
+        L.jf_rk3_stage_input.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.jf_rk3_stage_advance.restype = C.c_int
+        L.jf_rk3_stage_advance.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double]
         L.jf_set_tangent_seed.restype = C.c_int
         L.jf_set_tangent_seed.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.jf_rk3_step.restype = C.c_int
@@ -184,6 +199,9 @@ class Solver:
                 b.dirichlet = _dp(t)
             if fb.dist is not None:
                 b.dist = jf_disturbance(1, fb.dist["A"], fb.dist["kappa"], fb.dist["t1_lo"], fb.dist["t1_hi"])
+            if getattr(fb, "nb_width", None) is not None:
+                for d in range(3):
+                    b.nb_width[d] = float(fb.nb_width[d])
         ga = np.asarray(case.body_accel, dtype=np.float64)
         self._keep.append(ga)
         self.stream = stream
@@ -229,6 +247,32 @@ class Solver:
             dU = np.zeros_like(U) if dU0 is None else np.asarray(dU0)
             U = np.stack([U, dU], axis=-1)
         return self.torch.as_tensor(U, dtype=self.tdtype).contiguous().to(self.device)
+
+    # ---- block decomposition (include/jf.h "Block decomposition"); pointers are raw device addresses
+    def jf_fill_halo_axis(self, U_ptr, axis):
+        self._check(lib().jf_fill_halo_axis(self.h, C.c_void_p(U_ptr), int(axis)))
+
+    def jf_face_elems(self, face):
+        return int(lib().jf_face_elems(self.h, int(face)))
+
+    def jf_pack_face(self, U_ptr, face, buf):
+        self._check(lib().jf_pack_face(self.h, C.c_void_p(U_ptr), int(face), C.c_void_p(buf.data_ptr())))
+
+    def jf_unpack_face(self, U_ptr, face, buf):
+        self._check(lib().jf_unpack_face(self.h, C.c_void_p(U_ptr), int(face), C.c_void_p(buf.data_ptr())))
+
+    def jf_pull_face(self, U_ptr, face, peer_ptr, n_peer):
+        n = (C.c_int * 3)(*[int(v) for v in n_peer])
+        self._check(lib().jf_pull_face(self.h, C.c_void_p(U_ptr), int(face), C.c_void_p(peer_ptr), n))
+
+    def jf_rk3_stage_input(self, U, stage):
+        p = lib().jf_rk3_stage_input(self.h, self._ptr(U), int(stage))
+        if not p:
+            raise JFError(JF_EINVAL, "jf_rk3_stage_input")
+        return int(p)
+
+    def jf_rk3_stage_advance(self, U, stage, dt):
+        self._check(lib().jf_rk3_stage_advance(self.h, self._ptr(U), int(stage), float(dt)))
 
     def jf_set_tangent_seed(self, dA, dkappa):
         self._check(lib().jf_set_tangent_seed(self.h, float(dA), float(dkappa)))

@@ -13,7 +13,7 @@ from typing import List, Optional
 import numpy as np
 
 NH = 3
-BC_PERIODIC, BC_ZEROGRAD, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = range(5)
+BC_PERIODIC, BC_ZEROGRAD, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC, BC_EXCHANGE = range(6)
 
 
 @dataclass
@@ -23,6 +23,7 @@ class FaceBC:
     u_wall: tuple = (0.0, 0.0, 0.0)
     dirichlet: Optional[np.ndarray] = None   # prim[5][n_t2][n_t1] (rho,u,v,w,p)
     dist: Optional[dict] = None              # {"A","kappa","t1_lo","t1_hi"}  (Eq. 8)
+    nb_width: Optional[tuple] = None         # BC_EXCHANGE: widths of the neighbour block's 3 nearest cells
 
 
 @dataclass

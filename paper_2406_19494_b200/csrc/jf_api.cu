@@ -21,15 +21,18 @@ struct Metrics {
   std::vector<double> dl[3], xc[3], Xc[3], Xf[3];
 };
 
-void build_metrics(const int n[3], const double* const xf[3], const bool periodic[3], Metrics& M) {
+// nbw[f]: for a JF_BC_EXCHANGE face f, the widths of the neighbouring block's three cells next to the
+// face (nearest first) - the halo cells then have the geometry they have on the undivided grid; else null.
+void build_metrics(const int n[3], const double* const xf[3], const bool periodic[3], const double* const nbw[6],
+                   Metrics& M) {
   for (int a = 0; a < 3; ++a) {
     const int N = n[a], P = N + 2 * NH;
     std::vector<double>&d = M.dl[a], &x = M.xc[a];
     d.assign(P, 0.0); x.assign(P, 0.0); M.Xc[a].assign(P, 1.0); M.Xf[a].assign(P, 1.0);
     for (int i = 0; i < N; ++i) { d[i + NH] = xf[a][i + 1] - xf[a][i]; x[i + NH] = 0.5 * (xf[a][i] + xf[a][i + 1]); }
     for (int m = 1; m <= NH; ++m) {
-      d[NH - m] = periodic[a] ? d[NH + N - m] : d[NH + m - 1];
-      d[NH + N - 1 + m] = periodic[a] ? d[NH + m - 1] : d[NH + N - m];
+      d[NH - m] = nbw[2 * a] ? nbw[2 * a][m - 1] : (periodic[a] ? d[NH + N - m] : d[NH + m - 1]);
+      d[NH + N - 1 + m] = nbw[2 * a + 1] ? nbw[2 * a + 1][m - 1] : (periodic[a] ? d[NH + m - 1] : d[NH + N - m]);
     }
     double e = xf[a][0];
     for (int m = 1; m <= NH; ++m) { x[NH - m] = e - 0.5 * d[NH - m]; e -= d[NH - m]; }
@@ -190,8 +193,10 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
   const double* xf[3] = {g->xf, g->yf, g->zf};
   bool per[3];
   for (int a = 0; a < 3; ++a) per[a] = bc->face[2 * a].type == JF_BC_PERIODIC;
+  const double* nbw[6];
+  for (int f = 0; f < 6; ++f) nbw[f] = bc->face[f].type == JF_BC_EXCHANGE ? bc->face[f].nb_width : nullptr;
   Metrics M;
-  build_metrics(n, xf, per, M);
+  build_metrics(n, xf, per, nbw, M);
   Layout L = make_layout(n, sizeof(T));
   jf::Params<T>& P = I.P;
   for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
@@ -252,25 +257,59 @@ int pick_segment(long long warps_per_layer, int N) {
   return L < N ? L : N;
 }
 
+// boundary pass of one axis (both sides, 3 layers); JF_BC_EXCHANGE faces are left to the face transfer
 template <class T>
-jf_status launch_halo(jf_solver* s, Impl<T>& I, T* U) {
+jf_status launch_halo_axis(jf_solver* s, Impl<T>& I, T* U, int axis) {
   const jf::Params<T>& P = I.P;
-  {
-    Timed t(s, K_HALO);
+  Timed t(s, K_HALO);
+  if (axis == 0) {
     long long tot = (long long)P.n[1] * P.n[2] * 6;
     jf::halo_kernel<T, 0><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[0], I.bc[1], U);
-  }
-  {
-    Timed t(s, K_HALO);
+  } else if (axis == 1) {
     long long tot = (long long)P.P[0] * P.n[2] * 6;
     jf::halo_kernel<T, 1><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[2], I.bc[3], U);
-  }
-  {
-    Timed t(s, K_HALO);
+  } else {
     long long tot = (long long)P.P[0] * P.P[1] * 6;
     jf::halo_kernel<T, 2><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, I.bc[4], I.bc[5], U);
   }
-  s->launches += 3;
+  s->launches += 1;
+  JF_CUDA(s, cudaPeekAtLastError());
+  return JF_OK;
+}
+
+template <class T>
+jf_status launch_halo(jf_solver* s, Impl<T>& I, T* U) {
+  jf_status st;
+  for (int a = 0; a < 3; ++a)
+    if ((st = launch_halo_axis<T>(s, I, U, a))) return st;
+  return JF_OK;
+}
+
+// tangential cell counts of the boundary pass of `axis` (reading O3): x: interior (j,k); y: all padded i,
+// interior k; z: all padded (i,j)
+template <class T>
+long long face_cells(const jf::Params<T>& P, int axis) {
+  const long long n1 = axis == 0 ? P.n[1] : P.P[0], n2 = axis == 2 ? P.P[1] : P.n[2];
+  return n1 * n2;
+}
+
+// MODE 0 pack / 1 unpack / 2 pull of one face (jf_kernels.cuh: face_xfer_kernel)
+template <class T, int MODE>
+jf_status launch_xfer(jf_solver* s, Impl<T>& I, int face, T* U, T* buf, const T* peer, const int* np) {
+  const jf::Params<T>& P = I.P;
+  const int axis = face / 2, side = face % 2;
+  const long long tot = face_cells<T>(P, axis) * 3;
+  long long psy = 0, psz = 0, pvol = 0;
+  int Np = 0;
+  if (MODE == 2) {
+    psy = np[0] + 6; psz = psy * (np[1] + 6); pvol = psz * (np[2] + 6); Np = np[axis];
+  }
+  const unsigned blocks = (unsigned)((tot + 255) / 256);
+  Timed t(s, K_HALO);
+  if (axis == 0) jf::face_xfer_kernel<T, 0, MODE><<<blocks, 256, 0, s->stream>>>(P, side, U, buf, peer, Np, psy, psz, pvol);
+  else if (axis == 1) jf::face_xfer_kernel<T, 1, MODE><<<blocks, 256, 0, s->stream>>>(P, side, U, buf, peer, Np, psy, psz, pvol);
+  else jf::face_xfer_kernel<T, 2, MODE><<<blocks, 256, 0, s->stream>>>(P, side, U, buf, peer, Np, psy, psz, pvol);
+  s->launches += 1;
   JF_CUDA(s, cudaPeekAtLastError());
   return JF_OK;
 }
@@ -333,21 +372,28 @@ jf_status launch_rhs(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArg
   return s->viscous ? launch_rhs_t<T, true>(s, I, U, R, rk) : launch_rhs_t<T, false>(s, I, U, R, rk);
 }
 
+// SSP-RK3 (reading O8) stage by stage.  Stage input (the array whose halos must be filled): 1: U, 2: A, 3: B.
+//   1: A = U + dt L(U);  2: B = 3/4 U + 1/4 (A + dt L(A));  3: U = 1/3 U + 2/3 (B + dt L(B)) (pointwise in
+//   place: each thread reads U^n of its cell before writing it)
+template <class T>
+T* stage_input(Impl<T>& I, T* U, int stage) { return stage == 1 ? U : (stage == 2 ? I.A : I.B); }
+
+template <class T>
+jf_status stage_advance(jf_solver* s, Impl<T>& I, T* U, int stage, double dt) {
+  if (stage == 1) { jf::RKArgs<T> r{U, I.A, T(0), T(1), T(dt)}; return launch_rhs<T>(s, I, U, I.R, &r); }
+  if (stage == 2) { jf::RKArgs<T> r{U, I.B, T(0.75), T(0.25), T(dt)}; return launch_rhs<T>(s, I, I.A, I.R, &r); }
+  jf::RKArgs<T> r{U, U, T(1.0 / 3.0), T(2.0 / 3.0), T(dt)};
+  return launch_rhs<T>(s, I, I.B, I.R, &r);
+}
+
 template <class T>
 jf_status rk3(jf_solver* s, Impl<T>& I, T* U, double dt) {
   jf_status st;
-  // stage 1: A = U + dt L(U)
-  if ((st = launch_halo<T>(s, I, U))) return st;
-  jf::RKArgs<T> r1{U, I.A, T(0), T(1), T(dt)};
-  if ((st = launch_rhs<T>(s, I, U, I.R, &r1))) return st;
-  // stage 2: B = 3/4 U + 1/4 (A + dt L(A))
-  if ((st = launch_halo<T>(s, I, I.A))) return st;
-  jf::RKArgs<T> r2{U, I.B, T(0.75), T(0.25), T(dt)};
-  if ((st = launch_rhs<T>(s, I, I.A, I.R, &r2))) return st;
-  // stage 3: U = 1/3 U + 2/3 (B + dt L(B))   (pointwise in place: each thread reads U^n then writes)
-  if ((st = launch_halo<T>(s, I, I.B))) return st;
-  jf::RKArgs<T> r3{U, U, T(1.0 / 3.0), T(2.0 / 3.0), T(dt)};
-  return launch_rhs<T>(s, I, I.B, I.R, &r3);
+  for (int stage = 1; stage <= 3; ++stage) {
+    if ((st = launch_halo<T>(s, I, stage_input<T>(I, U, stage)))) return st;
+    if ((st = stage_advance<T>(s, I, U, stage, dt))) return st;
+  }
+  return JF_OK;
 }
 
 template <class T>
@@ -397,7 +443,8 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
     if ((bc->face[2 * a].type == JF_BC_PERIODIC) != (bc->face[2 * a + 1].type == JF_BC_PERIODIC)) return JF_EINVAL;
   for (int f = 0; f < 6; ++f) {
     const jf_bc_face& b = bc->face[f];
-    if ((int)b.type < 0 || (int)b.type > 4) return JF_EINVAL;
+    if ((int)b.type < 0 || (int)b.type > 5) return JF_EINVAL;
+    if (b.type == JF_BC_EXCHANGE && !(b.nb_width[0] > 0.0 && b.nb_width[1] > 0.0 && b.nb_width[2] > 0.0)) return JF_EINVAL;
     if (b.type == JF_BC_DIRICHLET && !b.dirichlet) return JF_EINVAL;
     if (b.type == JF_BC_WALL_ISOTHERMAL && !(b.T_wall > 0.0)) return JF_EINVAL;
   }
@@ -508,6 +555,67 @@ jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host)
   return s->dtype == JF_F64   ? cfl<double>(s, s->d, (const double*)U, cflnum, dt_host)
          : s->dtype == JF_F32 ? cfl<float>(s, s->f, (const float*)U, cflnum, dt_host)
                               : cfl<jf::Dual>(s, s->t, (const jf::Dual*)U, cflnum, dt_host);
+}
+
+// dispatch on the solver's scalar type: F(Impl<T>&, T tag)
+#define JF_DISPATCH(s, EXPR_D, EXPR_F, EXPR_T) \
+  ((s)->dtype == JF_F64 ? (EXPR_D) : (s)->dtype == JF_F32 ? (EXPR_F) : (EXPR_T))
+
+jf_status jf_fill_halo_axis(jf_solver* s, void* U, int axis) {
+  if (!s) return JF_EINVAL;
+  if (!U || axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_fill_halo_axis: null pointer or bad axis");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_fill_halo_axis: U not 16-byte aligned");
+  return JF_DISPATCH(s, launch_halo_axis<double>(s, s->d, (double*)U, axis), launch_halo_axis<float>(s, s->f, (float*)U, axis),
+                     launch_halo_axis<jf::Dual>(s, s->t, (jf::Dual*)U, axis));
+}
+
+size_t jf_face_elems(const jf_solver* s, int face) {
+  if (!s || face < 0 || face > 5) return 0;
+  return (size_t)(15 * JF_DISPATCH(s, face_cells<double>(s->d.P, face / 2), face_cells<float>(s->f.P, face / 2),
+                                   face_cells<jf::Dual>(s->t.P, face / 2)));
+}
+
+jf_status jf_pack_face(jf_solver* s, const void* U, int face, void* buf) {
+  if (!s) return JF_EINVAL;
+  if (!U || !buf || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_pack_face: null pointer or bad face");
+  return JF_DISPATCH(s, (launch_xfer<double, 0>(s, s->d, face, (double*)U, (double*)buf, nullptr, nullptr)),
+                     (launch_xfer<float, 0>(s, s->f, face, (float*)U, (float*)buf, nullptr, nullptr)),
+                     (launch_xfer<jf::Dual, 0>(s, s->t, face, (jf::Dual*)U, (jf::Dual*)buf, nullptr, nullptr)));
+}
+
+jf_status jf_unpack_face(jf_solver* s, void* U, int face, const void* buf) {
+  if (!s) return JF_EINVAL;
+  if (!U || !buf || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_unpack_face: null pointer or bad face");
+  return JF_DISPATCH(s, (launch_xfer<double, 1>(s, s->d, face, (double*)U, (double*)buf, nullptr, nullptr)),
+                     (launch_xfer<float, 1>(s, s->f, face, (float*)U, (float*)buf, nullptr, nullptr)),
+                     (launch_xfer<jf::Dual, 1>(s, s->t, face, (jf::Dual*)U, (jf::Dual*)buf, nullptr, nullptr)));
+}
+
+jf_status jf_pull_face(jf_solver* s, void* U, int face, const void* U_peer, const int n_peer[3]) {
+  if (!s) return JF_EINVAL;
+  if (!U || !U_peer || !n_peer || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_pull_face: null pointer or bad face");
+  const int a = face / 2;
+  const int* n = JF_DISPATCH(s, s->d.P.n, s->f.P.n, s->t.P.n);
+  for (int b = 0; b < 3; ++b)
+    if (n_peer[b] < 4 || (b != a && n_peer[b] != n[b]))
+      return fail(s, JF_EINVAL, "jf_pull_face: the peer block must match this block's tangential extents");
+  return JF_DISPATCH(s, (launch_xfer<double, 2>(s, s->d, face, (double*)U, nullptr, (const double*)U_peer, n_peer)),
+                     (launch_xfer<float, 2>(s, s->f, face, (float*)U, nullptr, (const float*)U_peer, n_peer)),
+                     (launch_xfer<jf::Dual, 2>(s, s->t, face, (jf::Dual*)U, nullptr, (const jf::Dual*)U_peer, n_peer)));
+}
+
+void* jf_rk3_stage_input(jf_solver* s, void* U, int stage) {
+  if (!s || !U || stage < 1 || stage > 3) return nullptr;
+  return JF_DISPATCH(s, (void*)stage_input<double>(s->d, (double*)U, stage), (void*)stage_input<float>(s->f, (float*)U, stage),
+                     (void*)stage_input<jf::Dual>(s->t, (jf::Dual*)U, stage));
+}
+
+jf_status jf_rk3_stage_advance(jf_solver* s, void* U, int stage, double dt) {
+  if (!s) return JF_EINVAL;
+  if (!U || stage < 1 || stage > 3 || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_stage_advance: bad argument");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_stage_advance: U not 16-byte aligned");
+  return JF_DISPATCH(s, stage_advance<double>(s, s->d, (double*)U, stage, dt), stage_advance<float>(s, s->f, (float*)U, stage, dt),
+                     stage_advance<jf::Dual>(s, s->t, (jf::Dual*)U, stage, dt));
 }
 
 jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {

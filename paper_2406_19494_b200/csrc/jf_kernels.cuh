@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, F
   long long str[3] = {1, P.sy, P.sz};
   long long tang = (long long)p1 * str[t1a] + (long long)p2 * str[t2a];
   long long og = tang + (long long)g * str[AXIS];
+  if (f.type == 5) return;      // JF_BC_EXCHANGE: filled from the neighbouring block (face_xfer_kernel)
   if (f.type == 0 || f.type == 1) {
     int src = f.type == 0 ? (side == 0 ? N - m : m - 1) : (side == 0 ? 0 : N - 1);
     long long os = tang + (long long)(src + NH) * str[AXIS];
@@ -115,6 +116,52 @@ __global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, F
   U[2 * P.vol + og] = W[0] * W[2];
   U[3 * P.vol + og] = W[0] * W[3];
   U[4 * P.vol + og] = W[4] / gas.gm1 + T(0.5) * W[0] * (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+}
+
+// ------------------------------------------------------------------ a1 across blocks: face transfer
+// Block decomposition (equal blocks [N/S + 2Nh], halo exchange "each device sends to
+// and receives from exactly one other device").  A face of type JF_BC_EXCHANGE takes its three halo
+// layers from the interior layers of the neighbouring block next to that face, over the same tangential
+// extents as the boundary pass of that axis (x: interior (j,k); y: all padded i; z: all padded (i,j)), so
+// that the x -> y -> z order defines edges and corners exactly as on the undivided grid.
+//   MODE 0 pack:   buf[q][m-1][a2][a1] <- the layer the neighbour across `side` needs (low side: m-1, high: N-m)
+//   MODE 1 unpack: halo layer m at `side` <- buf[q][m-1][a2][a1] (packed by the neighbour for its opposite side)
+//   MODE 2 pull:   halo layer m at `side` <- the peer block's state array directly (same device or a
+//                  peer-mapped NVLink address): low side reads peer layer Np-m, high side peer layer m-1
+template <class T, int AXIS, int MODE>
+__global__ void __launch_bounds__(256)
+face_xfer_kernel(Params<T> P, int side, T* U, T* buf, const T* __restrict__ peer, int Np, long long psy, long long psz,
+                 long long pvol) {
+  constexpr int t1a = (AXIS == 0) ? 1 : 0, t2a = (AXIS == 2) ? 1 : 2;
+  const int lo1 = (AXIS == 0) ? NH : 0, n1 = (AXIS == 0) ? P.n[1] : P.P[0];
+  const int lo2 = (AXIS == 2) ? 0 : NH, n2 = (AXIS == 2) ? P.P[1] : P.n[2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long per = (long long)n1 * n2, total = per * 3;
+  if (tid >= total) return;
+  int a1, a2, m;
+  if (AXIS == 0) { m = (int)(tid % 3) + 1; a1 = (int)((tid / 3) % n1); a2 = (int)(tid / (3LL * n1)); }
+  else { a1 = (int)(tid % n1); a2 = (int)((tid / n1) % n2); m = (int)(tid / per) + 1; }
+  const int p1 = lo1 + a1, p2 = lo2 + a2, N = P.n[AXIS];
+  const long long str[3] = {1, P.sy, P.sz};
+  const long long tang = (long long)p1 * str[t1a] + (long long)p2 * str[t2a];
+  const long long bo = ((long long)(m - 1) * n2 + a2) * n1 + a1;
+  if (MODE == 0) {
+    const long long os = tang + (long long)((side == 0 ? m - 1 : N - m) + NH) * str[AXIS];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) buf[q * total + bo] = U[q * P.vol + os];
+  } else {
+    const long long og = tang + (long long)((side == 0 ? -m : N - 1 + m) + NH) * str[AXIS];
+    if (MODE == 1) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q * P.vol + og] = buf[q * total + bo];
+    } else {
+      const long long pstr[3] = {1, psy, psz};
+      const long long os = (long long)p1 * pstr[t1a] + (long long)p2 * pstr[t2a] +
+                           (long long)((side == 0 ? Np - m : m - 1) + NH) * pstr[AXIS];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q * P.vol + og] = peer[q * pvol + os];
+    }
+  }
 }
 
 // ------------------------------------------------------------------ a5 (part) centre gradients
