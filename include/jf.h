@@ -166,6 +166,16 @@ jf_status jf_pull_face(jf_solver *s, void *U_dev, int face, const void *U_peer_d
 void *jf_rk3_stage_input(jf_solver *s, void *U_dev, int stage);
 jf_status jf_rk3_stage_advance(jf_solver *s, void *U_dev, int stage, double dt);
 
+/* ---- Plane statistics (Fig. 1: profiles averaged over the two homogeneous directions) --
+ * For every interior plane p of `axis` (0 x, 1 y, 2 z) the area-weighted sums over the plane's interior cells,
+ *   sums_dev[q * n_axis + p] = sum_{t1,t2} phi_q dA,   dA = Delta_t1 Delta_t2,
+ * of the JF_NSTATS quantities  phi = 1, rho, T, u, v, w, uu, vv, ww, uv, uw, vw, rho^2, T^2  (T = p/(rho R)).
+ * The caller forms means S_q/S_0 and Reynolds stresses <u_i u_j> - <u_i><u_j>.  sums_dev: DEVICE array of
+ * JF_NSTATS * n_axis doubles (double for every solver dtype; tangent solvers: value parts).  Deterministic
+ * (fixed reduction order for a given grid).  Asynchronous on the solver's stream. */
+#define JF_NSTATS 14
+jf_status jf_plane_sums(jf_solver *s, const void *U_dev, int axis, double *sums_dev);
+
 /* Tangent solvers (JF_F64_TANGENT) only; JF_EINVAL otherwise.  The paper introduces the Disturbance
  * Wall so that its parameters can be differentiated through the solver.
  * Sets the direction (dA, dkappa) in the parameter space of Eq. 8 (:112), applied to every disturbance

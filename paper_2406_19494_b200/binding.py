@@ -45,7 +45,7 @@ class jf_bc(C.Structure):
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
            "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
-           "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
+           "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_version"]
 
 _lib = None
@@ -92,6 +92,8 @@ def lib():
         L.jf_rk3_stage_input.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.jf_rk3_stage_advance.restype = C.c_int
         L.jf_rk3_stage_advance.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double]
+        L.jf_plane_sums.restype = C.c_int
+        L.jf_plane_sums.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.jf_set_tangent_seed.restype = C.c_int
         L.jf_set_tangent_seed.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.jf_rk3_step.restype = C.c_int
@@ -273,6 +275,12 @@ class Solver:
 
     def jf_rk3_stage_advance(self, U, stage, dt):
         self._check(lib().jf_rk3_stage_advance(self.h, self._ptr(U), int(stage), float(dt)))
+
+    def jf_plane_sums(self, U, axis):
+        """[JF_NSTATS = 14][n_axis] float64 device tensor of the area-weighted plane sums (include/jf.h)."""
+        out = self.torch.empty((14, self.case.n[axis]), dtype=self.torch.float64, device=self.device)
+        self._check(lib().jf_plane_sums(self.h, self._ptr(U), int(axis), C.c_void_p(out.data_ptr())))
+        return out
 
     def jf_set_tangent_seed(self, dA, dkappa):
         self._check(lib().jf_set_tangent_seed(self.h, float(dA), float(dkappa)))

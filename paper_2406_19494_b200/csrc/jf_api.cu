@@ -1,5 +1,6 @@
 // jf_api.cu — C ABI of libjf (include/jf.h): argument validation, metric / BC tables, workspace
 // carving, kernel launches.  Host logic only; every step of the path runs in jf_kernels.cuh.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -15,6 +16,7 @@ namespace {
 using jf::NH;
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+constexpr int STATS_NB = 16;  // at most this many partial blocks per plane in jf_plane_sums
 
 // Grid geometry (reading O2): widths, centres, halo geometry, index-space metrics.
 struct Metrics {
@@ -48,6 +50,7 @@ struct Layout {  // byte offsets into the workspace
   size_t tab_xc[3];     // double
   size_t dirichlet[6];  // double
   size_t cfl;           // 4 x u64
+  size_t stats;         // NSTAT x max(n) x STATS_NB doubles (plane-sum partials)
   size_t R, A, B, G;    // fields (dtype)
   size_t total;
 };
@@ -64,6 +67,7 @@ Layout make_layout(const int n[3], size_t esz) {
     L.dirichlet[f] = off; off = align_up(off + (size_t)5 * n[t1] * n[t2] * sizeof(double));
   }
   L.cfl = off; off = align_up(off + 4 * sizeof(unsigned long long));
+  L.stats = off; off = align_up(off + (size_t)jf::NSTAT * std::max(n[0], std::max(n[1], n[2])) * STATS_NB * sizeof(double));
   size_t vol = (size_t)(n[0] + 6) * (n[1] + 6) * (n[2] + 6);
   L.R = off; off = align_up(off + 5 * vol * esz);
   L.A = off; off = align_up(off + 5 * vol * esz);
@@ -89,6 +93,7 @@ struct Impl {
   jf::FaceBC<T> bc[6];
   T *R, *A, *B, *G;
   unsigned long long* cfl_out;
+  double* stats;
 };
 
 bool dtype_ok(jf_dtype d) { return d == JF_F64 || d == JF_F32 || d == JF_F64_TANGENT; }
@@ -236,6 +241,7 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
   }
   I.R = (T*)(ws + L.R); I.A = (T*)(ws + L.A); I.B = (T*)(ws + L.B); I.G = (T*)(ws + L.G);
   I.cfl_out = (unsigned long long*)(ws + L.cfl);
+  I.stats = (double*)(ws + L.stats);
   return JF_OK;
 }
 
@@ -417,6 +423,22 @@ jf_status cfl(jf_solver* s, Impl<T>& I, const T* U, double cflnum, double* dt_ho
   double dt = v[0];
   if (s->viscous) dt = std::fmin(dt, std::fmin((3.0 / 14.0) * v[1], (1.0 / 10.0) * v[2]));
   *dt_host = cflnum * dt;
+  return JF_OK;
+}
+
+template <class T>
+jf_status plane_sums(jf_solver* s, Impl<T>& I, const T* U, int axis, double* out) {
+  const jf::Params<T>& P = I.P;
+  const int np = P.n[axis];
+  const long long ntang = (long long)P.n[(axis + 1) % 3] * P.n[(axis + 2) % 3];
+  int NB = (int)std::min<long long>(STATS_NB, std::max<long long>(1, std::min<long long>((148LL * 8 + np - 1) / np, (ntang + 1023) / 1024)));
+  const dim3 grid(np, NB);
+  if (axis == 0) jf::plane_sums_kernel<T, 0><<<grid, 256, 0, s->stream>>>(P, U, I.stats, NB);
+  else if (axis == 1) jf::plane_sums_kernel<T, 1><<<grid, 256, 0, s->stream>>>(P, U, I.stats, NB);
+  else jf::plane_sums_kernel<T, 2><<<grid, 256, 0, s->stream>>>(P, U, I.stats, NB);
+  jf::plane_sums_final<<<(jf::NSTAT * np + 127) / 128, 128, 0, s->stream>>>(I.stats, out, np, NB);
+  s->launches += 2;
+  JF_CUDA(s, cudaPeekAtLastError());
   return JF_OK;
 }
 
@@ -616,6 +638,14 @@ jf_status jf_rk3_stage_advance(jf_solver* s, void* U, int stage, double dt) {
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_stage_advance: U not 16-byte aligned");
   return JF_DISPATCH(s, stage_advance<double>(s, s->d, (double*)U, stage, dt), stage_advance<float>(s, s->f, (float*)U, stage, dt),
                      stage_advance<jf::Dual>(s, s->t, (jf::Dual*)U, stage, dt));
+}
+
+jf_status jf_plane_sums(jf_solver* s, const void* U, int axis, double* sums) {
+  if (!s) return JF_EINVAL;
+  if (!U || !sums || axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_plane_sums: null pointer or bad axis");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_plane_sums: U not 16-byte aligned");
+  return JF_DISPATCH(s, plane_sums<double>(s, s->d, (const double*)U, axis, sums), plane_sums<float>(s, s->f, (const float*)U, axis, sums),
+                     plane_sums<jf::Dual>(s, s->t, (const jf::Dual*)U, axis, sums));
 }
 
 jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {

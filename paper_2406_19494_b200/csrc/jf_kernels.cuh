@@ -517,6 +517,64 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
   }
 }
 
+// ------------------------------------------------------------------ plane statistics
+// The paper's channel validation plots plane-averaged profiles over the two homogeneous directions: mean
+// density, temperature, velocity and Reynolds stresses (Fig. 1).  Per plane p of `AXIS`
+// (interior index) this forms the area-weighted sums  S_q(p) = sum_{t1,t2} phi_q dA,  dA = Delta_t1 Delta_t2,
+// over the interior cells of the plane, for the NSTAT quantities
+//   1, rho, T, u, v, w, uu, vv, ww, uv, uw, vw, rho^2, T^2
+// (mean = S_q / S_0; <u_i'u_j'> = <u_i u_j> - <u_i><u_j>: formed by the caller).  Accumulated in double for
+// every solver dtype.  Deterministic: block b of plane p reduces a fixed chunk with a fixed shuffle tree
+// into part[(q n_planes + p) NB + b]; plane_sums_final adds the NB partials in order.
+constexpr int NSTAT = 14;
+template <class T, int AXIS>
+__global__ void __launch_bounds__(256) plane_sums_kernel(Params<T> P, const T* __restrict__ U, double* __restrict__ part, int NB) {
+  constexpr int t1a = (AXIS == 0) ? 1 : 0, t2a = (AXIS == 2) ? 1 : 2;
+  const int p = blockIdx.x, b = blockIdx.y;
+  const int n1 = P.n[t1a], n2 = P.n[t2a];
+  const long long ntang = (long long)n1 * n2, chunk = (ntang + NB - 1) / NB;
+  const long long lo = b * chunk, hi = (lo + chunk < ntang) ? lo + chunk : ntang;
+  const long long str[3] = {1, P.sy, P.sz};
+  const Gas<T> gas = P.gas;
+  double acc[NSTAT];
+#pragma unroll
+  for (int q = 0; q < NSTAT; ++q) acc[q] = 0.0;
+  for (long long t = lo + threadIdx.x; t < hi; t += blockDim.x) {
+    const int a1 = (int)(t % n1), a2 = (int)(t / n1);
+    const long long o = (long long)(p + NH) * str[AXIS] + (long long)(a1 + NH) * str[t1a] + (long long)(a2 + NH) * str[t2a];
+    T W[6];
+    cons_to_prim<T>(gas, U[o], U[P.vol + o], U[2 * P.vol + o], U[3 * P.vol + o], U[4 * P.vol + o], W);
+    const double dA = (double)P.dl[t1a][a1 + NH] * (double)P.dl[t2a][a2 + NH];
+    const double r = (double)W[0], u = (double)W[1], v = (double)W[2], w = (double)W[3], Tt = (double)W[5];
+    const double f[NSTAT] = {1.0, r, Tt, u, v, w, u * u, v * v, w * w, u * v, u * w, v * w, r * r, Tt * Tt};
+#pragma unroll
+    for (int q = 0; q < NSTAT; ++q) acc[q] = fma(f[q], dA, acc[q]);
+  }
+  __shared__ double sred[8][NSTAT];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+  for (int q = 0; q < NSTAT; ++q) {
+    double a = acc[q];
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) a += __shfl_xor_sync(0xffffffffu, a, s);
+    if (lane == 0) sred[warp][q] = a;
+  }
+  __syncthreads();
+  if (threadIdx.x < NSTAT) {
+    double a = 0.0;
+    for (int wq = 0; wq < 8; ++wq) a += sred[wq][threadIdx.x];
+    part[((long long)threadIdx.x * gridDim.x + p) * NB + b] = a;
+  }
+}
+
+__global__ void plane_sums_final(const double* __restrict__ part, double* __restrict__ out, int nplanes, int NB) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;        // (q, p) flattened
+  if (i >= NSTAT * nplanes) return;
+  double a = 0.0;
+  for (int b = 0; b < NB; ++b) a += part[(long long)i * NB + b];
+  out[i] = a;
+}
+
 // ------------------------------------------------------------------ diagnostics: one face flux per thread
 // W[f][6 cells][6 prims] (cells i-2..i+3), Gt[f][4 cells][4] (cells i-1..i+2), Xf[f] -> F[f][5] of
 // the face i+1/2: per-cell WENO of cell i (W^-) and of cell i+1 (W^+), then the face flux —
