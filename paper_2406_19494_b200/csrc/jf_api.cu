@@ -161,6 +161,7 @@ void fill_gas(jf::Gas<T>& G, double gamma, double R_gas, double Pr, const jf_mu_
   G.lam_fac = T(gamma * R_gas / (gamma - 1.0) / Pr); G.Pr = T(Pr);
   G.sutherland = mu->sutherland != 0; G.viscous = mu->mu_ref > 0.0;
   for (int a = 0; a < 3; ++a) G.g[a] = T(ga ? ga[a] : 0.0);
+  G.has_g = ga && (ga[0] != 0.0 || ga[1] != 0.0 || ga[2] != 0.0);
 }
 
 template <class T>
@@ -327,8 +328,8 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
   const T* G = VISC ? I.G : nullptr;
   if (VISC) {
     Timed t(s, K_GRAD);
-    dim3 grid((P.P[0] + 255) / 256, P.P[1], P.P[2]);
-    jf::gradient_kernel<T><<<grid, 256, 0, s->stream>>>(P, U, I.G);
+    dim3 grid((P.P[0] + jf::GR_BX - 1) / jf::GR_BX, (P.P[1] + jf::GR_BY - 1) / jf::GR_BY, (P.P[2] + jf::GR_BZ - 1) / jf::GR_BZ);
+    jf::gradient_kernel<T><<<grid, dim3(jf::GR_BX, jf::GR_BY, jf::GR_BZ), 0, s->stream>>>(P, U, I.G);
     s->launches += 1;
   }
   {
@@ -337,7 +338,7 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
     const size_t sh = (size_t)jf::XS_WARPS * jf::XS<VISC>::NV * jf::XS_RING * sizeof(T);
     jf::sweep_x_kernel<T, VISC><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
-  const size_t sh = (size_t)jf::YZ_RING * jf::YZ<VISC>::NV * jf::YZ_TX * jf::YZ_TY * sizeof(T);
+  const size_t sh = (size_t)jf::YZ_RING * jf::YZ<VISC>::NP * jf::YZ_TX * jf::YZ_TY * sizeof(jf::Pair2<T>);
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
   jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0)};
   {
@@ -362,7 +363,7 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
 // 128-thread block in fp64): above the 48 KB default, so opt in once per solver.
 template <class T, bool VISC>
 cudaError_t opt_in_smem() {
-  const int sh = (int)((size_t)jf::YZ_RING * jf::YZ<VISC>::NV * jf::YZ_TX * jf::YZ_TY * sizeof(T));
+  const int sh = (int)((size_t)jf::YZ_RING * jf::YZ<VISC>::NP * jf::YZ_TX * jf::YZ_TY * sizeof(jf::Pair2<T>));
   cudaError_t e = cudaSuccess;
   auto set = [&](const void* f) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);

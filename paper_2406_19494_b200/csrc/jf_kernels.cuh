@@ -167,11 +167,17 @@ face_xfer_kernel(Params<T> P, int side, T* U, T* buf, const T* __restrict__ peer
 // ------------------------------------------------------------------ a5 (part) centre gradients
 // G[3*axis+comp] = D^c_axis u_comp, 4th order, difference form; written where the index along
 // `axis` is interior (all padded indices along the other two axes).
+#ifndef JF_GR_BX
+#define JF_GR_BX 32
+#define JF_GR_BY 4
+#define JF_GR_BZ 2
+#endif
+constexpr int GR_BX = JF_GR_BX, GR_BY = JF_GR_BY, GR_BZ = JF_GR_BZ;
 template <class T>
-__global__ void __launch_bounds__(256) gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G) {
-  const int pi = blockIdx.x * blockDim.x + threadIdx.x;
-  const int pj = blockIdx.y, pk = blockIdx.z;
-  if (pi >= P.P[0]) return;
+__global__ void __launch_bounds__(GR_BX * GR_BY * GR_BZ) gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G) {
+  const int pi = blockIdx.x * GR_BX + threadIdx.x;
+  const int pj = blockIdx.y * GR_BY + threadIdx.y, pk = blockIdx.z * GR_BZ + threadIdx.z;
+  if (pi >= P.P[0] || pj >= P.P[1] || pk >= P.P[2]) return;
   const long long o = (long long)pk * P.sz + (long long)pj * P.sy + pi;
   const long long str[3] = {1, P.sy, P.sz};
   const int pidx[3] = {pi, pj, pk};
@@ -193,6 +199,11 @@ __global__ void __launch_bounds__(256) gradient_kernel(Params<T> P, const T* __r
       G[(long long)(3 * a + c) * P.vol + o] = (T(8) * (vel[2][c] - vel[1][c]) - (vel[3][c] - vel[0][c])) * sc;
   }
 }
+
+// Two window values of one cell stored side by side, so that one 128-bit (fp64) shared-memory access
+// moves both: (rho,u) (v,w) (p,T) (g0,g1) (g2,g3).
+template <class T>
+struct alignas(sizeof(T) >= 8 ? 16 : 2 * sizeof(T)) Pair2 { T a, b; };
 
 template <class T>
 struct RKArgs {
@@ -292,9 +303,15 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     auto w = [&](int m, int q) -> T { return ring[q * XS_RING + ((tc + m) & (XS_RING - 1))]; };
     auto g = [&](int m, int c) -> T { return ring[(6 + c) * XS_RING + ((tc + m) & (XS_RING - 1))]; };
     T Wm[5], Wp[5];
+#ifdef JF_XS_BRANCHY
 #pragma unroll
     for (int q = 0; q < 5; ++q) { Wm[q] = T(1); Wp[q] = T(1); }
     if (cell) weno_cell_states<T, 0>(w, Wm, Wp);
+#else
+    // no divergent branch: lanes without a WENO cell compute on whatever the ring holds (no traps on
+    // the device) and their values are never used by a lane that writes
+    weno_cell_states<T, 0>(w, Wm, Wp);
+#endif
     // W^-_{pc-1/2} comes from lane-1; lane 0 takes lane 31's value of the previous iteration
     T WL[5];
 #pragma unroll
@@ -303,8 +320,12 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
       WmOld[q] = Wm[q];
     }
     T F[5] = {T(0), T(0), T(0), T(0), T(0)};
+#ifdef JF_XS_BRANCHY
     if (cell && pc >= 3)
       face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][pc - 1] : T(0), F);
+#else
+    face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][min(max(pc - 1, 0), Px - 1)] : T(0), F);
+#endif
     const bool upd = cell && pc >= 4;
     const T idl = upd ? P.inv_dl[0][pc - 1] : T(0);
 #pragma unroll
@@ -332,14 +353,19 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 #ifndef JF_YZ_TY
 #define JF_YZ_TY 4
 #endif
+#ifndef JF_YZ_PAIR_MASK
+#define JF_YZ_PAIR_MASK 3
+#endif
 constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY, YZ_RING = 5;
-template <bool VISC> struct YZ { static constexpr int NV = VISC ? 10 : 5; };
+template <bool VISC> struct YZ { static constexpr int NP = VISC ? 5 : 3; };   // pairs per window cell
 template <class T, int DIR, bool VISC, int MODE>
 __global__ void __launch_bounds__(YZ_TX * YZ_TY, JF_YZ_MINB)
 sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* R, RKArgs<T> rk, int L) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* ring = reinterpret_cast<T*>(smem_raw);  // [5 slots][NV][threads]
-  constexpr int NT = YZ_TX * YZ_TY, NV = YZ<VISC>::NV;
+  using P2 = Pair2<T>;
+  constexpr bool PAIR = (JF_YZ_PAIR_MASK >> MODE) & 1;   // window stored as pairs (128-bit accesses) or as scalars
+  P2* ring = reinterpret_cast<P2*>(smem_raw);  // [5 slots][NP pairs][threads]  (scalar: [5 slots][2 NP][threads])
+  constexpr int NT = YZ_TX * YZ_TY, NP = YZ<VISC>::NP;
   constexpr int OTH = (DIR == 1) ? 2 : 1;    // the non-marching, non-x axis
   const int tid = threadIdx.y * YZ_TX + threadIdx.x;
   const int ix = blockIdx.x * YZ_TX + threadIdx.x;
@@ -353,17 +379,29 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const T* gsrc[4] = {G + (long long)(3 * t1 + n) * P.vol + col, G + (long long)(3 * t1 + t1) * P.vol + col,
                       G + (long long)(3 * t2 + n) * P.vol + col, G + (long long)(3 * t2 + t2) * P.vol + col};
-  T* mine = ring + tid;
+  P2* mine = ring + tid;
+  T* mine1 = reinterpret_cast<T*>(smem_raw) + tid;
   auto put = [&](int slot, const T raw[5], const T gn[4]) {
     T W[6];
     cons_to_prim<T>(gas, raw[0], raw[1], raw[2], raw[3], raw[4], W);
-    T* dst = mine + slot * (NV * NT);
+    if (PAIR) {
+      P2* dst = mine + slot * (NP * NT);
+      dst[0] = P2{W[0], W[1]};
+      dst[NT] = P2{W[2], W[3]};
+      dst[2 * NT] = P2{W[4], W[5]};
+      if (VISC) {
+        dst[3 * NT] = P2{gn[0], gn[1]};
+        dst[4 * NT] = P2{gn[2], gn[3]};
+      }
+    } else {
+      T* dst = mine1 + slot * (2 * NP * NT);
 #pragma unroll
-    for (int q = 0; q < 5; ++q) dst[q * NT] = W[q];
-    if (VISC) {
-      dst[5 * NT] = W[5];
+      for (int q = 0; q < 5; ++q) dst[q * NT] = W[q];
+      if (VISC) {
+        dst[5 * NT] = W[5];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) dst[(6 + c) * NT] = gn[c];
+        for (int c = 0; c < 4; ++c) dst[(6 + c) * NT] = gn[c];
+      }
     }
   };
   T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
@@ -392,10 +430,18 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     {
       int s = s0;
 #pragma unroll
-      for (int m = 0; m < YZ_RING; ++m) { slot[m] = s * (NV * NT); s = (s == YZ_RING - 1) ? 0 : s + 1; }
+      for (int m = 0; m < YZ_RING; ++m) { slot[m] = s * (NP * NT); s = (s == YZ_RING - 1) ? 0 : s + 1; }
     }
-    auto w = [&](int m, int q) -> T { return mine[slot[m + 2] + q * NT]; };
-    auto g = [&](int m, int cc) -> T { return mine[slot[m + 2] + (6 + cc) * NT]; };
+    auto w = [&](int m, int q) -> T {
+      if (!PAIR) return mine1[2 * slot[m + 2] + q * NT];
+      const P2 v = mine[slot[m + 2] + (q >> 1) * NT];
+      return (q & 1) ? v.b : v.a;
+    };
+    auto g = [&](int m, int cc) -> T {
+      if (!PAIR) return mine1[2 * slot[m + 2] + (6 + cc) * NT];
+      const P2 v = mine[slot[m + 2] + (3 + (cc >> 1)) * NT];
+      return (cc & 1) ? v.b : v.a;
+    };
     T Wm[5], Wp[5];
     weno_cell_states<T, DIR>(w, Wm, Wp);
     // issue the loads this step consumes at its end
@@ -417,7 +463,7 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       for (int q = 0; q < 5; ++q) Rold[q] = R[q * P.vol + o];
       if (MODE == 2) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { un[q] = rk.Un[q * P.vol + o]; us[q] = U[q * P.vol + o]; }
+        for (int q = 0; q < 5; ++q) un[q] = rk.Un[q * P.vol + o];
       }
     }
     if (c >= c0) {                           // face c-1/2
@@ -428,12 +474,16 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
         T Rv[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - Fprev[q]) * idl;
-        if (MODE >= 1) {
+        if (MODE >= 1 && gas.has_g) {
           T rho = w(-1, 0), u = w(-1, 1), v = w(-1, 2), ww = w(-1, 3);
           Rv[1] += rho * gas.g[0]; Rv[2] += rho * gas.g[1]; Rv[3] += rho * gas.g[2];
           Rv[4] += rho * (u * gas.g[0] + v * gas.g[1] + ww * gas.g[2]);
         }
         if (MODE == 2) {
+          // U_s of cell c-1 entered the window four steps ago: an L1/L2 hit, loaded where it is used
+          // (loaded with the other arrays it costs the z sweep its last registers: spills)
+#pragma unroll
+          for (int q = 0; q < 5; ++q) us[q] = U[q * P.vol + o];
 #pragma unroll
           for (int q = 0; q < 5; ++q) rk.Uout[q * P.vol + o] = rk.a * un[q] + rk.b * (us[q] + rk.dt * Rv[q]);
         } else {

@@ -20,8 +20,20 @@
 
 namespace jf {
 
+// Double constants whose low mantissa word is not zero cannot be instruction immediates; as literals
+// they are re-materialised by pairs of uniform moves inside the loops.  Read from constant memory they
+// are direct operands of the FP64 instructions.
+enum { K_EPS4 = 0, K_13_3, K_SIXTH, K_THIRD, K_4_3, K_2_3, K_COUNT };
+#define JF_KVALS {4e-6, 13.0 / 3.0, 1.0 / 6.0, 1.0 / 3.0, 4.0 / 3.0, 2.0 / 3.0}
+static __constant__ double kConstD[K_COUNT] = JF_KVALS;
+
 template <class T> struct Num;
 template <> struct Num<double> {
+#ifdef JF_NO_KCONST
+  template <int I> static __device__ __forceinline__ double K() { constexpr double k[K_COUNT] = JF_KVALS; return k[I]; }
+#else
+  template <int I> static __device__ __forceinline__ double K() { return kConstD[I]; }
+#endif
   static __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
   // reciprocal for normal, finite a: hardware seed (MUFU.RCP64H, rel. error <= 2^-23) and one
   // cubic step x (1 + e + e^2), e = 1 - a x  =>  error ~ e^3 < 2^-66: a few ulp-fractions, not
@@ -46,6 +58,7 @@ template <> struct Num<double> {
   static __device__ __forceinline__ double abs_(double a) { return fabs(a); }
 };
 template <> struct Num<float> {
+  template <int I> static __device__ __forceinline__ float K() { constexpr double k[K_COUNT] = JF_KVALS; return float(k[I]); }
   static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
   // MUFU seeds (rel. error ~2^-22) refined by one Newton step: ~1 ulp, a fraction of the IEEE sequences
   static __device__ __forceinline__ float rcp(float a) {
@@ -68,6 +81,7 @@ template <> struct Num<float> {
 // tangent scalar: value part by the same formulas as Num<double>, tangent by the chain rule
 template <> struct Num<Dual> {
   using D = Num<double>;
+  template <int I> static __device__ __forceinline__ Dual K() { return Dual(kConstD[I]); }
   static __device__ __forceinline__ Dual fma_(Dual a, Dual b, Dual c) {
     return Dual(fma(a.v, b.v, c.v), fma(a.v, b.d, fma(a.d, b.v, c.d)));
   }
@@ -107,6 +121,7 @@ struct Gas {
   T lam_fac;                      // lambda = mu * lam_fac, lam_fac = cp/Pr = gamma R/((gamma-1) Pr)
   T Pr;
   int sutherland, viscous;
+  int has_g;                      // any non-zero body acceleration (Eq. 1 source)
   T g[3];
 };
 
@@ -133,49 +148,55 @@ __device__ __forceinline__ T viscosity(const Gas<T>& gas, T Tf) {
 //   vp = W^+_{i-1/2}: the right-biased value at face i-1/2 = weno(e,d,c,b,a).
 // Both use the same smoothness indicators beta_0(a,b,c), beta_1(b,c,d), beta_2(c,d,e): the
 // mirrored stencil swaps beta_0 <-> beta_2 and the linear weights (1,6,3)/10 <-> (3,6,1)/10.
-// Difference form: v = p1 + [w0 (p0-p1) + w2 (p2-p1)] / sum, with second differences A_k,
-//   vm: p0-p1 = (A0-A1)/3, p2-p1 = (A1-A2)/6;   vp: p0'-p1' = -(A1-A2)/3, p2'-p1' = -(A0-A1)/6,
-// weights as products of the other two e_k = (beta_k+eps)^2 (one reciprocal per value).
+// Everything is built from the first differences D1..D4 = b-a, c-b, d-c, e-d:
+//   second differences A0 = D2-D1, A1 = D3-D2, A2 = D4-D3;
+//   first-derivative parts of the indicators  a-4b+3c = A0+2 D2,  b-d = -(D2+D3),  3c-4d+e = A2-2 D3;
+//   candidates  p1 = c + D3/3 + D2/6,  p0-p1 = (A0-A1)/3,  p2-p1 = (A1-A2)/6  (mirrored: p1' = c - D2/3 - D3/6).
+// v = p1 + [w0 (p0-p1) + w2 (p2-p1)] / sum with the weights as products of the other two
+// e_k = (beta_k+eps)^2 (one reciprocal per value); with t1 = E12 (A0-A1), t2 = E01 (A1-A2):
+//   vm = c + D2/6 + [D3 + (t1 + 1.5 t2)/(E12 + 6 E02 + 3 E01)]/3,
+//   vp = c - D3/6 - [D2 + (1.5 t1 + t2)/(3 E12 + 6 E02 + E01)]/3.
 // Indicators are carried as 4*beta (eps scaled likewise), which leaves the weights unchanged.
+// 47 arithmetic instructions per variable and cell.
 template <class T>
 __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp) {
   using N = Num<T>;
-  const T eps4 = T(4e-6), c133 = T(13.0 / 3.0), sixth = T(1.0 / 6.0);
-  const T c30 = T(1.0 / 30.0), c20 = T(1.0 / 20.0);
-  T A0 = N::fma_(T(-2), b, a) + c, A1 = N::fma_(T(-2), c, b) + d, A2 = N::fma_(T(-2), d, c) + e;
-  T b0 = N::fma_(T(3), c, N::fma_(T(-4), b, a)), b1 = b - d, b2 = N::fma_(T(3), c, N::fma_(T(-4), d, e));
+  const T eps4 = N::template K<K_EPS4>(), c133 = N::template K<K_13_3>(), sixth = N::template K<K_SIXTH>(), third = N::template K<K_THIRD>();
+  T D1 = b - a, D2 = c - b, D3 = d - c, D4 = e - d;
+  T A0 = D2 - D1, A1 = D3 - D2, A2 = D4 - D3;
+  T b0 = N::fma_(T(2), D2, A0), b1 = D2 + D3, b2 = N::fma_(T(-2), D3, A2);
   T e0 = N::fma_(c133 * A0, A0, N::fma_(b0, b0, eps4));
   T e1 = N::fma_(c133 * A1, A1, N::fma_(b1, b1, eps4));
   T e2 = N::fma_(c133 * A2, A2, N::fma_(b2, b2, eps4));
   e0 *= e0; e1 *= e1; e2 *= e2;
   T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
   T t1 = E12 * (A0 - A1), t2 = E01 * (A1 - A2);
-  T mid = T(0.6) * E02;
   {  // face i+1/2: weights (0.1 E12, 0.6 E02, 0.3 E01)
-    T den = N::fma_(T(0.3), E01, N::fma_(T(0.1), E12, mid));
-    T num = N::fma_(c30, t1, c20 * t2);
-    T p1 = sixth * N::fma_(T(5), c, N::fma_(T(2), d, -b));
-    vm = N::fma_(num, N::rcp(den), p1);
+    T den = N::fma_(T(3), E01, N::fma_(T(6), E02, E12));
+    T num = N::fma_(T(1.5), t2, t1);
+    vm = N::fma_(third, N::fma_(num, N::rcp(den), D3), N::fma_(sixth, D2, c));
   }
   {  // face i-1/2: weights (0.3 E12, 0.6 E02, 0.1 E01)
-    T den = N::fma_(T(0.1), E01, N::fma_(T(0.3), E12, mid));
-    T num = N::fma_(c20, t1, c30 * t2);
-    T p1 = sixth * N::fma_(T(5), c, N::fma_(T(2), b, -d));
-    vp = N::fma_(-num, N::rcp(den), p1);
+    T den = N::fma_(T(3), E12, N::fma_(T(6), E02, E01));
+    T num = N::fma_(T(1.5), t1, t2);
+    vp = N::fma_(-third, N::fma_(num, N::rcp(den), D2), N::fma_(-sixth, D3, c));
   }
 }
 
-// HLLC flux in the rotated frame: states (rho, un, ut1, ut2, p) -> F = [mass, n, t1, t2, energy]
+// HLLC flux in the rotated frame: states (rho, un, ut1, ut2, p) -> F = [mass, n, t1, t2, energy].
+// H_K = (E_K + p_K)/rho_K is formed as c_K^2/(gamma-1) + q_K/2 (the same quantity for an ideal gas), so
+// that E is needed on the selected side only; the tangential momentum fluxes of the closed form,
+// rho un ut + S (fac ut - rho ut), equal ut times the mass flux.
 template <class T>
 __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const T R[5], T F[5]) {
   using N = Num<T>;
   T tL = N::rsqrt_(L[0]), tR = N::rsqrt_(R[0]);        // 1/sqrt(rho)
   T sL = L[0] * tL, sR = R[0] * tR;                      // sqrt(rho)
   T riL = tL * tL, riR = tR * tR;                        // 1/rho
-  T cL = N::sqrt_(gas.gamma * L[4]) * tL, cR = N::sqrt_(gas.gamma * R[4]) * tR;
-  T qL = L[1] * L[1] + L[2] * L[2] + L[3] * L[3], qR = R[1] * R[1] + R[2] * R[2] + R[3] * R[3];
-  T EL = L[4] * gas.inv_gm1 + T(0.5) * L[0] * qL, ER = R[4] * gas.inv_gm1 + T(0.5) * R[0] * qR;
-  T HL = (EL + L[4]) * riL, HR = (ER + R[4]) * riR;
+  T aL = gas.gamma * L[4] * riL, aR = gas.gamma * R[4] * riR;   // c^2
+  T cL = aL * N::rsqrt_(aL), cR = aR * N::rsqrt_(aR);
+  T hL = T(0.5) * (L[1] * L[1] + L[2] * L[2] + L[3] * L[3]), hR = T(0.5) * (R[1] * R[1] + R[2] * R[2] + R[3] * R[3]);
+  T HL = N::fma_(aL, gas.inv_gm1, hL), HR = N::fma_(aR, gas.inv_gm1, hR);
   T rs = N::rcp(sL + sR);
   T wL = sL * rs, wR = sR * rs;
   T un = wL * L[1] + wR * R[1], u1 = wL * L[2] + wR * R[2], u2 = wL * L[3] + wR * R[3];
@@ -187,20 +208,20 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
   // side selected by sign(S*)  (S* == 0: both star fluxes are mathematically equal)
   bool left = Ss >= T(0);
   T rho = left ? L[0] : R[0], vn = left ? L[1] : R[1], v1 = left ? L[2] : R[2], v2 = left ? L[3] : R[3];
-  T p = left ? L[4] : R[4], E = left ? EL : ER, SK = left ? SL : SR, m = left ? mL : mR;
+  T p = left ? L[4] : R[4], hq = left ? hL : hR, SK = left ? SL : SR, m = left ? mL : mR;
   T ri = left ? riL : riR;
   T Sc = left ? N::min_(SL, T(0)) : N::max_(SR, T(0));  // min(S_L,0) / max(S_R,0)
+  T E = N::fma_(rho, hq, p * gas.inv_gm1);
   T mn = rho * vn;
-  T F0 = mn, F1 = mn * vn + p, F2 = mn * v1, F3 = mn * v2, F4 = vn * (E + p);
   T dinv = N::rcp(SK - Ss);
   T fac = m * dinv;
   T dS = Ss - vn;
   T Es = fac * (E * ri + dS * Ss) + dS * p * dinv;       // fac*(E/rho + dS*(S* + p/m))
-  F[0] = F0 + Sc * (fac - rho);
-  F[1] = F1 + Sc * (fac * Ss - mn);
-  F[2] = F2 + Sc * (fac * v1 - rho * v1);
-  F[3] = F3 + Sc * (fac * v2 - rho * v2);
-  F[4] = F4 + Sc * (Es - E);
+  F[0] = N::fma_(Sc, fac - rho, mn);
+  F[1] = N::fma_(Sc, N::fma_(fac, Ss, -mn), N::fma_(mn, vn, p));
+  F[2] = v1 * F[0];
+  F[3] = v2 * F[0];
+  F[4] = N::fma_(Sc, Es - E, vn * (E + p));
 }
 
 // Dissipative flux (Eq. 4-5, rotated frame) of the face between cells -1 | 0 along DIR, subtracted
@@ -212,25 +233,30 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
 template <class T, int DIR, class WAcc, class GAcc>
 __device__ __forceinline__ void viscous_sub(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T Fr[5]) {
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  T dn[4], fv[4];  // normal derivative and face value of u_n, u_t1, u_t2, T
+  // Unscaled stencil sums: dn = 24 X_xi^f * (normal derivative), fv = 16 * (face value), gt = 16 * (face
+  // interpolation of the transverse centre derivative) of u_n, u_t1, u_t2, T; the scale factors are folded
+  // into mX = mu/(24 X_xi^f) and mG = mu/16.
+  T dn[4], fv[4];
   constexpr int qv[4] = {1 + n, 1 + t1, 1 + t2, 5};
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     T m1 = w(-2, qv[c]), c0 = w(-1, qv[c]), p1 = w(0, qv[c]), p2 = w(1, qv[c]);
-    dn[c] = (T(27) * (p1 - c0) - (p2 - m1)) * i24Xf;
-    fv[c] = (T(9) * (c0 + p1) - (m1 + p2)) * T(1.0 / 16.0);
+    dn[c] = Num<T>::fma_(T(27), p1 - c0, m1 - p2);
+    fv[c] = Num<T>::fma_(T(9), c0 + p1, -(m1 + p2));
   }
   T gt[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c)
-    gt[c] = (T(9) * (g(-1, c) + g(0, c)) - (g(-2, c) + g(1, c))) * T(1.0 / 16.0);
-  T mu = viscosity<T>(gas, fv[3]);
-  T div = dn[0] + gt[1] + gt[3];
-  T tnn = mu * (T(2) * dn[0] - T(2.0 / 3.0) * div);
-  T tn1 = mu * (gt[0] + dn[1]);
-  T tn2 = mu * (gt[2] + dn[2]);
+    gt[c] = Num<T>::fma_(T(9), g(-1, c) + g(0, c), -(g(-2, c) + g(1, c)));
+  T mu = gas.sutherland ? viscosity<T>(gas, fv[3] * T(1.0 / 16.0)) : gas.mu_ref;
+  T mX = mu * i24Xf, mG = mu * T(1.0 / 16.0);
+  // tau_nn = mu (2 d_n u_n - 2/3 div) = mu (4/3 d_n u_n - 2/3 (d_t1 u_t1 + d_t2 u_t2))
+  T tnn = Num<T>::fma_(mX * Num<T>::template K<K_4_3>(), dn[0], -(mG * Num<T>::template K<K_2_3>()) * (gt[1] + gt[3]));
+  T tn1 = Num<T>::fma_(mX, dn[1], mG * gt[0]);
+  T tn2 = Num<T>::fma_(mX, dn[2], mG * gt[2]);
   Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
-  Fr[4] -= fv[0] * tnn + fv[1] * tn1 + fv[2] * tn2 + mu * gas.lam_fac * dn[3];
+  T work = Num<T>::fma_(fv[2], tn2, Num<T>::fma_(fv[1], tn1, fv[0] * tnn));
+  Fr[4] = Num<T>::fma_(-(mX * gas.lam_fac), dn[3], Num<T>::fma_(T(-1.0 / 16.0), work, Fr[4]));
 }
 
 // Rotated-frame component order of direction DIR: slot c of (rho, u_n, u_t1, u_t2, p) is
