@@ -4,7 +4,7 @@ pieces of one RHS, as an exact cubic in 1/n for an n^3 periodic box (Taylor-Gree
 
 The counts come from the oracle run on its counting scalar type (ora_count_flops_*); they are
 polynomial in 1/n because the work is (n+6)^3 cons->prim conversions, 3 n^2 (n+1) faces and n^3
-cells.  Calls only oracle/ and the input generators.  Usage: python oracle/count_flops.py
+cells; plus the count of one step of config 2 (channel) at full size.  Calls only oracle/ and the input generators.  Usage: python oracle/count_flops.py
 """
 import json
 import os
@@ -36,6 +36,12 @@ def main():
              "columns": ["basic", "div", "sqrt", "total"], "fit_sizes": sizes}
     for k, v in rows.items():
         model[k] = np.linalg.solve(V, np.array(v)).T.tolist()     # [column][coefficient]
+    # config 2 (channel 192x128x128: walls, Sutherland viscosity, body force): counted at full size
+    c = cases.channel()
+    o = ora.Oracle(c)
+    model["channel_step"] = (o.count_flops_step(o.state(), 1e-4) / c.cells).tolist()
+    model["channel_dims"] = list(c.n)
+    print("channel flops per cell-step:", model["channel_step"][3], flush=True)
     with open(os.path.join(ROOT, "oracle", "flop_model.json"), "w") as f:
         json.dump(model, f, indent=1)
     print("asymptotic flops per cell-step:", model["step"][3][0])
