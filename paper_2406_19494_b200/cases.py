@@ -203,7 +203,9 @@ def _sutherland(T, mu_ref, T_ref, S):
 def blasius_compressible(M, Pr, gamma, T_inf, Tw_over_Tinf, mu_law, eta_max=8.0, n_eta=1601):
     """Compressible Blasius similarity solve (Eq. 7): (C f'')' + f f'' = 0,
     (C g'/Pr)' + f g' + C (gamma-1) M^2 f''^2 = 0, C = rho mu/(rho_e mu_e), f(0)=f'(0)=0,
-    g(0)=T_w/T_inf, f'(inf)=g(inf)=1; RK4 + damped-Newton shooting.  Input generation only."""
+    g(0)=T_w/T_inf (isothermal wall) or, with Tw_over_Tinf=None, g'(0)=0 (adiabatic wall, g(0) found),
+    f'(inf)=g(inf)=1; RK4 + damped-Newton shooting.  Input generation only."""
+    adiabatic = Tw_over_Tinf is None
     mu_e = _sutherland(T_inf, **mu_law)
 
     def Cfun(g):
@@ -219,7 +221,8 @@ def blasius_compressible(M, Pr, gamma, T_inf, Tw_over_Tinf, mu_law, eta_max=8.0,
     d = eta[1] - eta[0]
 
     def integrate(a, b):
-        y = np.array([0.0, 0.0, a, Tw_over_Tinf, b])
+        # unknowns: a = C f''(0) and b = (C/Pr) g'(0) (isothermal) or b = g(0) (adiabatic)
+        y = np.array([0.0, 0.0, a, b, 0.0]) if adiabatic else np.array([0.0, 0.0, a, Tw_over_Tinf, b])
         out = np.empty((n_eta, 5))
         out[0] = y
         for n in range(1, n_eta):
@@ -232,7 +235,7 @@ def blasius_compressible(M, Pr, gamma, T_inf, Tw_over_Tinf, mu_law, eta_max=8.0,
         o = integrate(a, b)
         return np.array([o[-1, 1] - 1.0, o[-1, 3] - 1.0])
 
-    x = np.array([0.5, 4.0])
+    x = np.array([0.5, 1.0 + 0.5 * np.sqrt(Pr) * (gamma - 1.0) * M * M]) if adiabatic else np.array([0.5, 4.0])
     r = resid(*x)
     for _ in range(60):
         if np.max(np.abs(r)) < 1e-11:
@@ -246,7 +249,7 @@ def blasius_compressible(M, Pr, gamma, T_inf, Tw_over_Tinf, mu_law, eta_max=8.0,
         while lam > 1e-4:
             xn = x + lam * step
             with np.errstate(all="ignore"):
-                rn = resid(*xn) if xn[0] > 0 else np.array([np.inf, np.inf])
+                rn = resid(*xn) if xn[0] > 0 and (not adiabatic or xn[1] > 0) else np.array([np.inf, np.inf])
             if np.all(np.isfinite(rn)) and np.linalg.norm(rn) < np.linalg.norm(r):
                 break
             lam *= 0.5
@@ -305,6 +308,57 @@ def flat_plate(nx=512, ny=192, nz=8, cfl=0.5, n_steps=200, A_frac=0.01, disturba
 
 
 # ------------------------------------------------------------------ parity / edge-case inputs
+def paper_boundary_layer(nx=300, ny=200, nz=4, cfl=0.5, n_steps=20, A=0.01, kappa=10.0, disturbance=True):
+    """The paper's own section 3.2 case (parameters in tests/golden/paper_section_3_2.txt):
+    laminar compressible boundary layer, M = 2.25, Pr = 0.72, unit Reynolds number 1e4, (x, y) in
+    [1, 1.5] x [0, 0.4] on 300 x 200 cells, uniform in x, stretched in y (beta = 2.2), no-slip ADIABATIC south
+    wall carrying the Disturbance Wall v = A sin(2 pi kappa x) (Eq. 8, A = 0.01, kappa = 10) over its whole
+    length, zero-gradient north and east, self-similar (compressible Blasius, Eq. 7) profile at the west inlet.
+    Units: rho_e = u_e = T_e = 1, x measured from the leading edge (so that Re_x = 1e4 x).  Readings where the
+    paper is silent: R = 1/(gamma M^2); Sutherland with T_ref = T_e, mu_ref = mu_e = 1e-4, S = 110.4/273.15 T_e;
+    one-sided tanh map; nz spanwise cells of width dx, periodic; the local similarity profile at every x as the
+    initial field (v = w = 0)."""
+    gamma, M, Pr, Re_unit = 1.4, 2.25, 0.72, 1.0e4
+    Rg = 1.0 / (gamma * M * M)
+    mu_law = {"mu_ref": 1.0 / Re_unit, "T_ref": 1.0, "S": 110.4 / 273.15}
+    xf = uniform_faces(1.0, 1.0 + 0.5 * nx / 300.0, nx)            # dx fixed at 0.5/300 for reduced sizes
+    yf = tanh_faces_one_sided(ny, 2.2, 0.4)
+    dx = xf[1] - xf[0]
+    zf = uniform_faces(0.0, nz * dx, nz)
+    sim = blasius_compressible(M, Pr, gamma, 1.0, None, mu_law)
+    Ieta = np.concatenate(([0.0], np.cumsum(0.5 * (sim["g"][1:] + sim["g"][:-1]) * np.diff(sim["eta"]))))
+    xc, yc = centres(xf), centres(yf)
+
+    def profile(x):                                                 # Eq. 7 inverted: y(eta) at distance x
+        yeta = np.sqrt(2.0 * mu_law["mu_ref"] * x) * Ieta
+        return np.interp(yc, yeta, sim["fp"], right=1.0), np.interp(yc, yeta, sim["g"], right=1.0)
+
+    shp = (nz, ny, nx)
+    u, T = np.empty(shp), np.empty(shp)
+    for i, x in enumerate(xc):
+        up, Tp = profile(x)
+        u[:, :, i], T[:, :, i] = up[None, :], Tp[None, :]
+    p = np.full(shp, Rg)                                            # p_e = rho_e R T_e
+    zero = np.zeros(shp)
+    U = set_interior_from_prim(empty_state((nx, ny, nz)), gamma, p / (Rg * T), u, zero, zero, p)
+    u_in, T_in = profile(xf[0])
+    inflow = np.empty((5, nz, ny))
+    inflow[0] = (1.0 / T_in)[None, :]
+    inflow[1] = u_in[None, :]
+    inflow[2] = 0.0
+    inflow[3] = 0.0
+    inflow[4] = Rg
+    bc = periodic_bc()
+    bc[0] = FaceBC(BC_DIRICHLET, dirichlet=inflow)
+    bc[1] = FaceBC(BC_ZEROGRAD)
+    dist = {"A": A, "kappa": kappa, "t1_lo": xf[0], "t1_hi": xf[-1]} if disturbance else None
+    bc[2] = FaceBC(BC_WALL_ADIABATIC, dist=dist)
+    bc[3] = FaceBC(BC_ZEROGRAD)
+    return Case(name=f"paperbl{nx}x{ny}x{nz}", n=(nx, ny, nz), xf=xf, yf=yf, zf=zf, gamma=gamma, R_gas=Rg, Pr=Pr,
+                mu=dict(sutherland=1, **mu_law), bc=bc, U0=U, cfl=cfl, n_steps=n_steps,
+                notes={"M": M, "Tw_over_Te": sim["h0"], "s0": sim["s0"], "blasius_resid": sim["resid"]})
+
+
 def random_admissible(n=(12, 10, 8), seed=1, bc=None, viscous=True, stretched=False, amp=0.3):
     """Seeded random admissible state (rho > 0, p > 0) with distinct per-cell values."""
     rng = np.random.default_rng(seed)

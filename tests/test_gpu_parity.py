@@ -254,6 +254,31 @@ def test_config3_flat_plate_full_size_5_steps(jf, ora):
     assert np.all(err <= TOL["f64"]), err
 
 
+def test_paper_section_3_2_boundary_layer_with_disturbance_wall(jf, ora):
+    # the paper's own case (tests/golden/paper_section_3_2.txt): 300 x 200 cells, adiabatic
+    # Disturbance Wall A = 0.01, kappa = 10 over the whole south wall, similarity inflow, zero-gradient N/E
+    c = cases.paper_boundary_layer(n_steps=20)
+    o = ora.Oracle(c)
+    s = jf.Solver(c, "f64")
+    Ug, Uo = s.jf_fill_halo(s.state()).cpu().numpy(), o.fill_halo(o.state())
+    assert np.array_equal(Ug[INT], Uo[INT])
+    scale = np.max(np.abs(Uo), axis=(1, 2, 3), keepdims=True)
+    scale[1:4] = np.max(scale[1:4])                            # rho v, rho w are ~0 here: scale by the momentum
+    assert np.max(np.abs(Ug - Uo) / scale) <= 1e-13             # every halo cell
+    err, rel_dt, Ug, Uo = run_both(jf, ora, c)
+    assert rel_dt <= 1e-12
+    band = sensitivity_band(ora, c, Uo)
+    print("paper 3.2 case, 20 steps: gpu-vs-oracle", err, "oracle fma-vs-nofma", band)
+    assert np.all(err <= np.maximum(TOL["f64"], BAND_FACTOR * band)), (err, band)
+    assert np.all(err[[0, 1, 4]] <= TOL["f64"]), err
+    # A = 0 is the plain no-slip wall on the GPU path as well, bit for bit after 3 steps
+    a = cases.paper_boundary_layer(nx=60, ny=40, A=0.0)
+    b = cases.paper_boundary_layer(nx=60, ny=40, disturbance=False)
+    Ua, _ = jf.run_case(a, "f64", n_steps=3)
+    Ub, _ = jf.run_case(b, "f64", n_steps=3)
+    assert np.array_equal(Ua.cpu().numpy(), Ub.cpu().numpy())
+
+
 def test_config4_tgv64_20_steps(jf, ora):
     err, _, _, _ = run_both(jf, ora, cases.tgv(64, n_steps=20))
     assert np.all(err <= TOL["f64"]), err
