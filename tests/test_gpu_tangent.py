@@ -155,6 +155,40 @@ def test_tangent_on_the_mach6_flat_plate_config(jf, ora):
     assert np.max(np.abs(tan[3])) <= 1e-15 * np.max(np.abs(fd[1]))
 
 
+@pytest.mark.parametrize("which", ["A", "kappa"])
+def test_tangent_on_the_papers_own_case(jf, ora, which):
+    """The paper's section 3.2 case with its printed A = 0.01, kappa = 10 (tests/golden/paper_section_3_2.txt) on
+    the first 150 x 60 cells of its grid: dU/dA and dU/dkappa after 10 steps against central differences of the
+    oracle, and the derivative of a scalar objective (the wall-normal momentum in the first cell row: what an
+    end-to-end optimisation of the disturbance, would descend on)."""
+    c = cases.paper_boundary_layer(nx=150, ny=60, nz=4)
+    d = c.bc[2].dist
+    o = ora.Oracle(c, "f64")
+    st, dt = o.cfl_dt(o.fill_halo(o.state()), 0.5)
+    n_steps = 10
+    key = "A" if which == "A" else "kappa"
+    h = 1e-5 * d[key]
+    cp, cm = copy.deepcopy(c), copy.deepcopy(c)
+    cp.bc[2].dist[key] = d[key] + h
+    cm.bc[2].dist[key] = d[key] - h
+    Up, Um = oracle_run(ora, cp, dt, n_steps), oracle_run(ora, cm, dt, n_steps)
+    fd = ((Up - Um) / (2 * h))[INT]
+    s = jf.Solver(c, "f64t")
+    s.jf_set_tangent_seed(1.0 if which == "A" else 0.0, 1.0 if which == "kappa" else 0.0)
+    U = s.state()
+    for _ in range(n_steps):
+        s.jf_rk3_step(U, dt)
+    tan = U.cpu().numpy()[..., 1][INT]
+    err = [float(np.max(np.abs(tan[q] - fd[q])) / np.max(np.abs(fd[q]))) for q in (0, 1, 2, 4)]
+    print("paper case dU/d" + which, "vs oracle central differences (rho, rho u, rho v, E):", err)
+    assert max(err) <= 1e-5, err
+    J = lambda V: float(np.sum(V[2][:, 0, :] ** 2))           # sum over the first cell row of (rho v)^2
+    dJ_fd = (J(Up[INT]) - J(Um[INT])) / (2 * h)
+    val = U.cpu().numpy()[..., 0][INT]
+    dJ_tan = float(np.sum(2.0 * val[2][:, 0, :] * tan[2][:, 0, :]))
+    assert dJ_fd != 0.0 and abs(dJ_tan - dJ_fd) <= 1e-6 * abs(dJ_fd), (dJ_tan, dJ_fd)
+
+
 def test_seed_rejected_on_plain_solvers(jf):
     c = wall_case()
     s = jf.Solver(c, "f64")
