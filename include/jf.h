@@ -58,7 +58,8 @@ typedef enum {
 
 /* Grid: face coordinates per axis (host pointers, copied by jf_create), strictly increasing.
  * Stretched meshes (:31, :104) are given through these arrays; Delta x_{i,j,k} of Eq. 6 is
- * xf[i+1]-xf[i].  Each n >= 4. */
+ * xf[i+1]-xf[i].  Each n >= 4, and (nx+6)(ny+6)(nz+6) < 2^32 (cells of one variable are addressed with a
+ * 32-bit offset; a 1600^3 box is 33 GB per variable, beyond one GPU anyway); otherwise JF_EINVAL. */
 typedef struct {
   int nx, ny, nz;
   const double *xf, *yf, *zf; /* nx+1, ny+1, nz+1 entries */

@@ -84,6 +84,8 @@ bool grid_ok(const jf_grid* g) {
   for (int a = 0; a < 3; ++a)
     for (int i = 0; i < n[a]; ++i)
       if (!(xf[a][i + 1] > xf[a][i])) return false;
+  // the kernels address a cell inside one variable's array with a 32-bit offset
+  if ((double)(g->nx + 6) * (double)(g->ny + 6) * (double)(g->nz + 6) >= 4294967296.0) return false;
   return true;
 }
 

@@ -372,13 +372,15 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   const int io = blockIdx.y * YZ_TY + threadIdx.y;
   const int N = P.n[DIR];
   if (ix >= P.n[0] || io >= P.n[OTH]) return;
-  const long long sm = (DIR == 1) ? P.sy : P.sz, so = (DIR == 1) ? P.sz : P.sy;
-  const long long col = (long long)(io + NH) * so + (ix + NH);
+  // in-plane element offsets fit 32 bits (jf_create checks vol < 2^32); the variable planes are addressed as
+  // uniform base + 32-bit offset: one address instruction per access instead of a 64-bit add
+  const unsigned sm = (unsigned)((DIR == 1) ? P.sy : P.sz), so = (unsigned)((DIR == 1) ? P.sz : P.sy);
+  const unsigned col = (unsigned)(io + NH) * so + (unsigned)(ix + NH);
   const int c0 = blockIdx.z * L, c1 = min(c0 + L, N);
   const Gas<T> gas = P.gas;
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  const T* gsrc[4] = {G + (long long)(3 * t1 + n) * P.vol + col, G + (long long)(3 * t1 + t1) * P.vol + col,
-                      G + (long long)(3 * t2 + n) * P.vol + col, G + (long long)(3 * t2 + t2) * P.vol + col};
+  const T* gsrc[4] = {G + (long long)(3 * t1 + n) * P.vol, G + (long long)(3 * t1 + t1) * P.vol,
+                      G + (long long)(3 * t2 + n) * P.vol, G + (long long)(3 * t2 + t2) * P.vol};
   P2* mine = ring + tid;
   T* mine1 = reinterpret_cast<T*>(smem_raw) + tid;
   auto put = [&](int slot, const T raw[5], const T gn[4]) {
@@ -411,11 +413,11 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     T raws[YZ_RING][5], gns[YZ_RING][4];
 #pragma unroll
     for (int s = 0; s < YZ_RING; ++s) {
-      const long long o = col + (long long)(c0 + s) * sm;
+      const unsigned o = col + (unsigned)(c0 + s) * sm;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raws[s][q] = U[q * P.vol + o];
+      for (int q = 0; q < 5; ++q) raws[s][q] = (U + q * P.vol)[o];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) gns[s][c] = VISC ? gsrc[c][(long long)(c0 + s) * sm] : T(0);
+      for (int c = 0; c < 4; ++c) gns[s][c] = VISC ? gsrc[c][o] : T(0);
     }
 #pragma unroll
     for (int s = 0; s < YZ_RING; ++s) put(s, raws[s], gns[s]);
@@ -424,8 +426,14 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
 #pragma unroll
   for (int q = 0; q < 5; ++q) { WmPrev[q] = T(1); Fprev[q] = T(0); }
   int s0 = 0;                                // slot of cell c-2
+  // metric table entries of the face / cell the NEXT step treats, loaded one step ahead (a per-step
+  // scalar load issued where it is used stalls the warp for an L2 round trip: 11-13 % of all stall samples)
+  T xf_n = VISC ? P.i24Xf[DIR][c0 - 1 + NH - 1] : T(0), idl_n = P.inv_dl[DIR][c0 - 1 + NH - 1];
   for (int c = c0 - 1; c <= c1; ++c) {
     const int pc = c + NH;
+    const T xf_c = xf_n, idl_c = idl_n;      // 1/(24 X_xi^f) of face c-1/2, 1/Delta of cell c-1
+    xf_n = VISC ? P.i24Xf[DIR][pc] : T(0);
+    idl_n = P.inv_dl[DIR][pc];
     int slot[YZ_RING];
     {
       int s = s0;
@@ -447,30 +455,30 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     // issue the loads this step consumes at its end
     const bool more = c < c1;                // another cell follows: its window needs padded pc+3
     const bool upd = c > c0;                 // cell c-1 is in [c0, c1): update it
-    const long long o = col + (long long)(pc - 1) * sm;
+    const unsigned o = col + (unsigned)(pc - 1) * sm;
     T Rold[5], un[5], us[5];
     if (more) {
-      const long long on = col + (long long)(pc + 3) * sm;
+      const unsigned on = col + (unsigned)(pc + 3) * sm;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raw[q] = U[q * P.vol + on];
+      for (int q = 0; q < 5; ++q) raw[q] = (U + q * P.vol)[on];
       if (VISC) {
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) gn[cc] = gsrc[cc][(long long)(pc + 3) * sm];
+        for (int cc = 0; cc < 4; ++cc) gn[cc] = gsrc[cc][on];
       }
     }
     if (upd) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) Rold[q] = R[q * P.vol + o];
+      for (int q = 0; q < 5; ++q) Rold[q] = (R + q * P.vol)[o];
       if (MODE == 2) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) un[q] = rk.Un[q * P.vol + o];
+        for (int q = 0; q < 5; ++q) un[q] = (rk.Un + q * P.vol)[o];
       }
     }
     if (c >= c0) {                           // face c-1/2
       T F[5];
-      face_flux<T, DIR, VISC>(gas, WmPrev, Wp, w, g, VISC ? P.i24Xf[DIR][pc - 1] : T(0), F);
+      face_flux<T, DIR, VISC>(gas, WmPrev, Wp, w, g, xf_c, F);
       if (upd) {
-        const T idl = P.inv_dl[DIR][pc - 1];
+        const T idl = idl_c;
         T Rv[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - Fprev[q]) * idl;
@@ -483,12 +491,12 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
           // U_s of cell c-1 entered the window four steps ago: an L1/L2 hit, loaded where it is used
           // (loaded with the other arrays it costs the z sweep its last registers: spills)
 #pragma unroll
-          for (int q = 0; q < 5; ++q) us[q] = U[q * P.vol + o];
+          for (int q = 0; q < 5; ++q) us[q] = (U + q * P.vol)[o];
 #pragma unroll
-          for (int q = 0; q < 5; ++q) rk.Uout[q * P.vol + o] = rk.a * un[q] + rk.b * (us[q] + rk.dt * Rv[q]);
+          for (int q = 0; q < 5; ++q) (rk.Uout + q * P.vol)[o] = rk.a * un[q] + rk.b * (us[q] + rk.dt * Rv[q]);
         } else {
 #pragma unroll
-          for (int q = 0; q < 5; ++q) R[q * P.vol + o] = Rv[q];
+          for (int q = 0; q < 5; ++q) (R + q * P.vol)[o] = Rv[q];
         }
       }
 #pragma unroll
