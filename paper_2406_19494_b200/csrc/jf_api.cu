@@ -252,6 +252,9 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
 // face and a window prologue, so segments should be long; but the grid must still fill the 148 SMs
 // (12 resident warps each) for several waves.  Largest power-of-two length (<= N) that leaves at
 // least JF_SEG_WAVES waves of warps, never below 8 cells.
+#ifndef JF_GM_WAVES
+#define JF_GM_WAVES 8
+#endif
 #ifndef JF_SEG_WAVES
 #define JF_SEG_WAVES 4
 #endif
@@ -330,8 +333,14 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
   const T* G = VISC ? I.G : nullptr;
   if (VISC) {
     Timed t(s, K_GRAD);
-    dim3 grid((P.P[0] + jf::GR_BX - 1) / jf::GR_BX, (P.P[1] + jf::GR_BY - 1) / jf::GR_BY, (P.P[2] + jf::GR_BZ - 1) / jf::GR_BZ);
-    jf::gradient_kernel<T><<<grid, dim3(jf::GR_BX, jf::GR_BY, jf::GR_BZ), 0, s->stream>>>(P, U, I.G);
+    // plane march: z segments long enough to amortise the 4-plane prologue, short enough for JF_GM_WAVES waves
+    const int tiles = ((P.P[0] + jf::GM_TX - 1) / jf::GM_TX) * ((P.P[1] + jf::GM_TY - 1) / jf::GM_TY);
+    int nseg = (JF_GM_WAVES * 148 * 4 + tiles - 1) / tiles;
+    if (nseg > P.P[2] / 8) nseg = P.P[2] / 8;
+    if (nseg < 1) nseg = 1;
+    const int Lz = (P.P[2] + nseg - 1) / nseg;
+    dim3 grid((P.P[0] + jf::GM_TX - 1) / jf::GM_TX, (P.P[1] + jf::GM_TY - 1) / jf::GM_TY, (P.P[2] + Lz - 1) / Lz);
+    jf::gradient_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
     s->launches += 1;
   }
   {
