@@ -313,8 +313,10 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   const int S = min(XS_LINES, rows - row0) * Px;            // stream length of this warp
   T* ring = reinterpret_cast<T*>(smem_raw) + warp * (NV * XS_RING);
   const Gas<T> gas = P.gas;
-  const long long gv[4] = {(long long)(3 * 1 + 0) * P.vol, (long long)(3 * 1 + 1) * P.vol,   // d_y u, d_y v
-                           (long long)(3 * 2 + 0) * P.vol, (long long)(3 * 2 + 2) * P.vol};  // d_z u, d_z w
+  // in-plane element offsets fit 32 bits (jf_create checks vol < 2^32): uniform plane base + 32-bit offset
+  const T* gsrc[4] = {G + (long long)(3 * 1 + 0) * P.vol, G + (long long)(3 * 1 + 1) * P.vol,   // d_y u, d_y v
+                      G + (long long)(3 * 2 + 0) * P.vol, G + (long long)(3 * 2 + 2) * P.vol};  // d_z u, d_z w
+  const unsigned usy = (unsigned)P.sy, uline = (unsigned)(P.sz - (long long)(ny - 1) * P.sy);
   const int kmax = (S - 1) / 32;             // last stream cell to treat: S-3 (pc = nx+3 of the last line)
   const unsigned full = 0xffffffffu;
   const int src_lane = (lane + 31) & 31;
@@ -324,21 +326,21 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     const int l = lane / Px, row = row0 + l;
     p = lane - l * Px; j = row % ny; k = row / ny;
   }
-  long long base = (long long)(k + NH) * P.sz + (long long)(j + NH) * P.sy;
+  unsigned base = (unsigned)(k + NH) * (unsigned)P.sz + (unsigned)(j + NH) * usy;
   auto advance = [&]() {                     // to the cell loaded in the next iteration
     p += 32;
     while (p >= Px) {
       p -= Px;
-      if (++j == ny) { j = 0; ++k; base += P.sz - (long long)(ny - 1) * P.sy; } else base += P.sy;
+      if (++j == ny) { j = 0; base += uline; } else base += usy;
     }
   };
   T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
   auto fetch = [&](bool in) {                // the cell at (base, p); `in`: inside this warp's stream
 #pragma unroll
-    for (int q = 0; q < 5; ++q) raw[q] = in ? U[q * P.vol + base + p] : T(1);
+    for (int q = 0; q < 5; ++q) raw[q] = in ? (U + q * P.vol)[base + (unsigned)p] : T(1);
     if (VISC) {
 #pragma unroll
-      for (int c = 0; c < 4; ++c) gn[c] = in ? G[gv[c] + base + p] : T(0);
+      for (int c = 0; c < 4; ++c) gn[c] = in ? gsrc[c][base + (unsigned)p] : T(0);
     }
   };
   fetch(lane < S);
@@ -361,7 +363,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     }
     // WENO cell of this lane: stream index t-2 = padded cell pc = p-2 of the same line (if p >= 4)
     const int pc = p - 2;
-    const long long cbase = base;
+    const unsigned cbase = base;
     const bool cell = t < S && p >= 4;       // 2 <= pc <= nx+3
     if (kc < kmax) { advance(); fetch(t + 32 < S); }
     __syncwarp();
@@ -394,11 +396,17 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 #endif
     const bool upd = cell && pc >= 4;
     const T idl = upd ? P.inv_dl[0][pc - 1] : T(0);
+    T dF[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       T Fm = shfl(full, lane == 31 ? Fold[q] : F[q], src_lane);
       Fold[q] = F[q];
-      if (upd) R[q * P.vol + cbase + pc - 1] = -(F[q] - Fm) * idl;
+      dF[q] = -(F[q] - Fm) * idl;
+    }
+    if (upd) {
+      const unsigned oc = cbase + (unsigned)(pc - 1);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) (R + q * P.vol)[oc] = dF[q];
     }
     __syncwarp();
   }
