@@ -346,7 +346,7 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
   {
     Timed t(s, K_SWEEP_X);
     const int groups = (P.n[1] * P.n[2] + jf::XS_LINES - 1) / jf::XS_LINES;   // one warp per group of lines
-    const size_t sh = (size_t)jf::XS_WARPS * jf::XS<VISC>::NV * jf::XS_RING * sizeof(T);
+    const size_t sh = (size_t)jf::XS_WARPS * (jf::XS<VISC>::NV * jf::XS_RING + jf::XS_CARRY) * sizeof(T);
     jf::sweep_x_kernel<T, VISC><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
   const size_t sh = (size_t)jf::YZ_RING * jf::YZ<VISC>::NP * jf::YZ_TX * jf::YZ_TY * sizeof(jf::Pair2<T>);

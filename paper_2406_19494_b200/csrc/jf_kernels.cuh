@@ -298,7 +298,7 @@ struct RKArgs {
 #ifndef JF_XS_LINES
 #define JF_XS_LINES 4
 #endif
-constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES;
+constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES, XS_CARRY = 10;
 template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, bool VISC>
 __global__ void __launch_bounds__(XS_WARPS * 32, JF_XS_MINB)
@@ -311,7 +311,8 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   const int row0 = (blockIdx.x * XS_WARPS + warp) * XS_LINES;
   if (row0 >= rows) return;
   const int S = min(XS_LINES, rows - row0) * Px;            // stream length of this warp
-  T* ring = reinterpret_cast<T*>(smem_raw) + warp * (NV * XS_RING);
+  T* ring = reinterpret_cast<T*>(smem_raw) + warp * (NV * XS_RING + XS_CARRY);
+  T* carry = ring + NV * XS_RING;            // W^- [5] and F [5] of lane 31, handed to lane 0 of the next iteration
   const Gas<T> gas = P.gas;
   // in-plane element offsets fit 32 bits (jf_create checks vol < 2^32): uniform plane base + 32-bit offset
   const T* gsrc[4] = {G + (long long)(3 * 1 + 0) * P.vol, G + (long long)(3 * 1 + 1) * P.vol,   // d_y u, d_y v
@@ -319,7 +320,6 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   const unsigned usy = (unsigned)P.sy, uline = (unsigned)(P.sz - (long long)(ny - 1) * P.sy);
   const int kmax = (S - 1) / 32;             // last stream cell to treat: S-3 (pc = nx+3 of the last line)
   const unsigned full = 0xffffffffu;
-  const int src_lane = (lane + 31) & 31;
   // this lane's load cell: stream index 32kc+lane = padded cell p of line (j,k), advanced by 32 per iteration
   int p, j, k;
   {
@@ -344,9 +344,11 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     }
   };
   fetch(lane < S);
-  T WmOld[5], Fold[5];                       // this lane's W^- and F of the previous iteration
+  if (lane == 31) {
 #pragma unroll
-  for (int q = 0; q < 5; ++q) { WmOld[q] = T(1); Fold[q] = T(0); }
+    for (int q = 0; q < 5; ++q) { carry[q] = T(1); carry[5 + q] = T(0); }
+  }
+  __syncwarp();
   for (int kc = 0; kc <= kmax; ++kc) {
     const int t = 32 * kc + lane;            // stream index of the loaded cell
     if (t < S) {
@@ -380,12 +382,12 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     // the device) and their values are never used by a lane that writes
     weno_cell_states<T, 0>(w, Wm, Wp);
 #endif
-    // W^-_{pc-1/2} comes from lane-1; lane 0 takes lane 31's value of the previous iteration
+    // W^-_{pc-1/2} comes from lane-1; lane 0 takes lane 31's value of the previous iteration (shared memory)
     T WL[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      WL[q] = shfl(full, lane == 31 ? WmOld[q] : Wm[q], src_lane);
-      WmOld[q] = Wm[q];
+      const T up = shfl_up(full, Wm[q], 1);
+      WL[q] = lane == 0 ? carry[q] : up;
     }
     T F[5] = {T(0), T(0), T(0), T(0), T(0)};
 #ifdef JF_XS_BRANCHY
@@ -399,9 +401,14 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     T dF[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      T Fm = shfl(full, lane == 31 ? Fold[q] : F[q], src_lane);
-      Fold[q] = F[q];
+      const T up = shfl_up(full, F[q], 1);
+      const T Fm = lane == 0 ? carry[5 + q] : up;
       dF[q] = -(F[q] - Fm) * idl;
+    }
+    __syncwarp();                            // lane 0 has read the carry of the previous iteration
+    if (lane == 31) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) { carry[q] = Wm[q]; carry[5 + q] = F[q]; }
     }
     if (upd) {
       const unsigned oc = cbase + (unsigned)(pc - 1);

@@ -104,6 +104,10 @@ template <class T> __device__ __forceinline__ T shfl(unsigned m, T a, int src) {
 __device__ __forceinline__ Dual shfl(unsigned m, Dual a, int src) {
   return Dual(__shfl_sync(m, a.v, src), __shfl_sync(m, a.d, src));
 }
+template <class T> __device__ __forceinline__ T shfl_up(unsigned m, T a, int d) { return __shfl_up_sync(m, a, d); }
+__device__ __forceinline__ Dual shfl_up(unsigned m, Dual a, int d) {
+  return Dual(__shfl_up_sync(m, a.v, d), __shfl_up_sync(m, a.d, d));
+}
 template <class T> __device__ __forceinline__ T shfl_xor(unsigned m, T a, int lm) { return __shfl_xor_sync(m, a, lm); }
 __device__ __forceinline__ Dual shfl_xor(unsigned m, Dual a, int lm) {
   return Dual(__shfl_xor_sync(m, a.v, lm), __shfl_xor_sync(m, a.d, lm));
