@@ -292,6 +292,12 @@ struct RKArgs {
 #ifndef JF_XS_WARPS
 #define JF_XS_WARPS 4
 #endif
+#ifndef JF_XS_MINB_F32
+#define JF_XS_MINB_F32 4
+#endif
+#ifndef JF_YZ_MINB_F32
+#define JF_YZ_MINB_F32 5
+#endif
 #ifndef JF_XS_MINB
 #define JF_XS_MINB 4
 #endif
@@ -301,7 +307,7 @@ struct RKArgs {
 constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES, XS_CARRY = 10;
 template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
 template <class T, bool VISC>
-__global__ void __launch_bounds__(XS_WARPS * 32, JF_XS_MINB)
+__global__ void __launch_bounds__(XS_WARPS * 32, sizeof(T) == 4 ? JF_XS_MINB_F32 : JF_XS_MINB)
 sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* __restrict__ R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_y v, d_z u, d_z w]
@@ -440,7 +446,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY, YZ_RING = 5;
 template <bool VISC> struct YZ { static constexpr int NP = VISC ? 5 : 3; };   // pairs per window cell
 template <class T, int DIR, bool VISC, int MODE>
-__global__ void __launch_bounds__(YZ_TX * YZ_TY, JF_YZ_MINB)
+__global__ void __launch_bounds__(YZ_TX * YZ_TY, sizeof(T) == 4 ? JF_YZ_MINB_F32 : JF_YZ_MINB)
 sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* R, RKArgs<T> rk, int L) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using P2 = Pair2<T>;

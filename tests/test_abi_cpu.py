@@ -56,6 +56,17 @@ def test_workspace_bytes(L):
     keep[0][3] = keep[0][2]                                   # non-monotone faces
     assert L.jf_workspace_bytes(C.byref(g), 0) == 0
     assert L.jf_workspace_bytes(C.byref(g), 7) == 0
+    # maximum size: cells of one variable are addressed with 32-bit offsets, (nx+6)(ny+6)(nz+6) < 2^32
+    def big(n):                                               # grid description only: no state is allocated
+        f = np.linspace(0.0, 1.0, n + 1)
+        gg = binding.jf_grid()
+        gg.nx = gg.ny = gg.nz = n
+        gg.xf = gg.yf = gg.zf = f.ctypes.data_as(C.POINTER(C.c_double))
+        return gg, f
+    g, keep = big(1618)                                        # 1624^3 = 4 283 098 624 < 2^32: accepted
+    assert L.jf_workspace_bytes(C.byref(g), 0) > 24 * 1624 ** 3 * 8
+    g, keep = big(1620)                                        # 1626^3 = 4 298 942 376 >= 2^32: refused
+    assert L.jf_workspace_bytes(C.byref(g), 0) == 0
 
 
 def test_create_validates_before_touching_the_device(L):
