@@ -165,13 +165,17 @@ face_xfer_kernel(Params<T> P, int side, T* U, T* buf, const T* __restrict__ peer
 }
 
 // Two window values of one cell stored side by side, so that one 128-bit (fp64) shared-memory access
-// moves both: (rho,u) (v,w) (p,T) (g0,g1) (g2,g3).
+// moves both: (rho,u) (v,w) (p,T) (g0,g1) (g2,-).
 template <class T>
 struct alignas(sizeof(T) >= 8 ? 16 : 2 * sizeof(T)) Pair2 { T a, b; };
 
 // ------------------------------------------------------------------ a5 (part) centre gradients
-// G[3*axis+comp] = D^c_axis u_comp, 4th order, difference form; written where the index along `axis` is
-// interior (all padded indices along the other two axes).  Plane march: a block owns a GM_TX x GM_TY tile of the (x,y) plane and marches along z
+// G[3*axis+comp] = D^c_axis u_comp (axis != comp), 4th order, difference form; written where the index along
+// `axis` is interior (all padded indices along the other two axes).  The diagonal slots hold the SUM of the other
+// two diagonal derivatives, G[4*n] = D^c_t1 u_t1 + D^c_t2 u_t2 (all tau_nn of the sweep along n needs; written where
+// both terms exist): a sweep reads 3 arrays instead of 4.  The sums with D^c_z w are formed two planes late, when the
+// z derivative is complete, from a two-deep thread-private shared-memory queue of d_x u and d_y v.
+// Plane march: a block owns a GM_TX x GM_TY tile of the (x,y) plane and marches along z
 // over the padded planes [k0, k1): per plane every thread converts its own cell (and the first threads the
 // cells of the 2-wide rim of the tile) to (u,v,w) ONCE and stores them in a double-buffered shared-memory
 // plane; the x and y derivatives of that plane are formed from shared memory, the z derivative of the plane
@@ -190,6 +194,11 @@ template <class T>
 __global__ void __launch_bounds__(GM_TX * GM_TY, sizeof(T) > 8 ? 1 : JF_GM_MINB)
 gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz) {
   __shared__ T sv[2][3][GM_SY][GM_SX];
+  // thread-private queue of (d_x u, d_y v) of planes p-2, p-1: shared memory (the registers are full at 3 blocks
+  // per SM), registers for the tangent type (one block per SM; its planes already fill the static 48 KB)
+  constexpr bool SQ = sizeof(T) <= 8;
+  __shared__ T sd[2][2][SQ ? GM_TX * GM_TY : 1];
+  T dq[2][2] = {{T(0), T(0)}, {T(0), T(0)}};
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * GM_TX + tx;
   const int x0 = blockIdx.x * GM_TX, y0 = blockIdx.y * GM_TY;
   const int px = x0 + tx, py = y0 + ty;
@@ -245,29 +254,46 @@ gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz)
     }
     __syncthreads();
     const unsigned op = o_own + (unsigned)p * sz;
+    T dxu = T(0), dyv = T(0);                  // the diagonal derivatives of plane p
     if (p >= k0 && p < k1) {
       if (dx_ok) {
+        T d[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
           const T* r = &sv[b][c][ty + 2][tx + 2];
-          (G + (long long)(0 + c) * P.vol)[op] = (T(8) * (r[1] - r[-1]) - (r[2] - r[-2])) * scx;
+          d[c] = (T(8) * (r[1] - r[-1]) - (r[2] - r[-2])) * scx;
         }
+        dxu = d[0];
+        (G + (long long)1 * P.vol)[op] = d[1];
+        (G + (long long)2 * P.vol)[op] = d[2];
       }
       if (dy_ok) {
+        T d[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
           const T* r = &sv[b][c][ty + 2][tx + 2];
-          (G + (long long)(3 + c) * P.vol)[op] = (T(8) * (r[GM_SX] - r[-GM_SX]) - (r[2 * GM_SX] - r[-2 * GM_SX])) * scy;
+          d[c] = (T(8) * (r[GM_SX] - r[-GM_SX]) - (r[2 * GM_SX] - r[-2 * GM_SX])) * scy;
         }
+        dyv = d[1];
+        (G + (long long)3 * P.vol)[op] = d[0];
+        (G + (long long)5 * P.vol)[op] = d[2];
       }
+      if (dx_ok && dy_ok) (G + (long long)8 * P.vol)[op] = dxu + dyv;
     }
     const int pzc = p - 2;                     // plane whose z derivative is complete now
     if (own && pzc >= k0 && pzc < k1 && pzc >= NH && pzc < P.n[2] + NH && p - 4 >= pstart) {
       const T scz = P.i12Xc[2][pzc];
+      T d[3];
 #pragma unroll
-      for (int c = 0; c < 3; ++c)
-        (G + (long long)(6 + c) * P.vol)[op - 2u * sz] = (T(8) * (q[3][c] - q[1][c]) - (q[4][c] - q[0][c])) * scz;
+      for (int c = 0; c < 3; ++c) d[c] = (T(8) * (q[3][c] - q[1][c]) - (q[4][c] - q[0][c])) * scz;
+      const unsigned oz = op - 2u * sz;
+      (G + (long long)6 * P.vol)[oz] = d[0];
+      (G + (long long)7 * P.vol)[oz] = d[1];
+      if (dy_ok) (G + (long long)0 * P.vol)[oz] = (SQ ? sd[b][1][tid] : dq[0][1]) + d[2];
+      if (dx_ok) (G + (long long)4 * P.vol)[oz] = d[2] + (SQ ? sd[b][0][tid] : dq[0][0]);
     }
+    if (SQ) { sd[b][0][tid] = dxu; sd[b][1][tid] = dyv; }   // slot p & 1 held plane p-2 until here
+    else { dq[0][0] = dq[1][0]; dq[0][1] = dq[1][1]; dq[1][0] = dxu; dq[1][1] = dyv; }
   }
 }
 
@@ -305,12 +331,12 @@ struct RKArgs {
 #define JF_XS_LINES 4
 #endif
 constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES, XS_CARRY = 10;
-template <bool VISC> struct XS { static constexpr int NV = VISC ? 10 : 5; };
+template <bool VISC> struct XS { static constexpr int NV = VISC ? 9 : 5; };
 template <class T, bool VISC>
 __global__ void __launch_bounds__(XS_WARPS * 32, sizeof(T) == 4 ? JF_XS_MINB_F32 : JF_XS_MINB)
 sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* __restrict__ R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_y v, d_z u, d_z w]
+  constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_z u, d_y v + d_z w]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ny = P.n[1], nz = P.n[2], nx = P.n[0], Px = P.P[0];
   const int rows = ny * nz;
@@ -321,8 +347,8 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   T* carry = ring + NV * XS_RING;            // W^- [5] and F [5] of lane 31, handed to lane 0 of the next iteration
   const Gas<T> gas = P.gas;
   // in-plane element offsets fit 32 bits (jf_create checks vol < 2^32): uniform plane base + 32-bit offset
-  const T* gsrc[4] = {G + (long long)(3 * 1 + 0) * P.vol, G + (long long)(3 * 1 + 1) * P.vol,   // d_y u, d_y v
-                      G + (long long)(3 * 2 + 0) * P.vol, G + (long long)(3 * 2 + 2) * P.vol};  // d_z u, d_z w
+  const T* gsrc[3] = {G + (long long)(3 * 1 + 0) * P.vol, G + (long long)(3 * 2 + 0) * P.vol,   // d_y u, d_z u
+                      G};                                                                       // d_y v + d_z w
   const unsigned usy = (unsigned)P.sy, uline = (unsigned)(P.sz - (long long)(ny - 1) * P.sy);
   const int kmax = (S - 1) / 32;             // last stream cell to treat: S-3 (pc = nx+3 of the last line)
   const unsigned full = 0xffffffffu;
@@ -340,13 +366,13 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
       if (++j == ny) { j = 0; base += uline; } else base += usy;
     }
   };
-  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
+  T raw[5], gn[3] = {T(0), T(0), T(0)};
   auto fetch = [&](bool in) {                // the cell at (base, p); `in`: inside this warp's stream
 #pragma unroll
     for (int q = 0; q < 5; ++q) raw[q] = in ? (U + q * P.vol)[base + (unsigned)p] : T(1);
     if (VISC) {
 #pragma unroll
-      for (int c = 0; c < 4; ++c) gn[c] = in ? gsrc[c][base + (unsigned)p] : T(0);
+      for (int c = 0; c < 3; ++c) gn[c] = in ? gsrc[c][base + (unsigned)p] : T(0);
     }
   };
   fetch(lane < S);
@@ -366,7 +392,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
       if (VISC) {
         dst[5 * XS_RING] = W[5];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) dst[(6 + c) * XS_RING] = gn[c];
+        for (int c = 0; c < 3; ++c) dst[(6 + c) * XS_RING] = gn[c];
       }
     }
     // WENO cell of this lane: stream index t-2 = padded cell pc = p-2 of the same line (if p >= 4)
@@ -466,11 +492,11 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   const int c0 = blockIdx.z * L, c1 = min(c0 + L, N);
   const Gas<T> gas = P.gas;
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  const T* gsrc[4] = {G + (long long)(3 * t1 + n) * P.vol, G + (long long)(3 * t1 + t1) * P.vol,
-                      G + (long long)(3 * t2 + n) * P.vol, G + (long long)(3 * t2 + t2) * P.vol};
+  const T* gsrc[3] = {G + (long long)(3 * t1 + n) * P.vol, G + (long long)(3 * t2 + n) * P.vol,   // d_t1 u_n, d_t2 u_n
+                      G + (long long)(4 * n) * P.vol};                                            // d_t1 u_t1 + d_t2 u_t2
   P2* mine = ring + tid;
   T* mine1 = reinterpret_cast<T*>(smem_raw) + tid;
-  auto put = [&](int slot, const T raw[5], const T gn[4]) {
+  auto put = [&](int slot, const T raw[5], const T gn[3]) {
     T W[6];
     cons_to_prim<T>(gas, raw[0], raw[1], raw[2], raw[3], raw[4], W);
     if (PAIR) {
@@ -480,7 +506,7 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       dst[2 * NT] = P2{W[4], W[5]};
       if (VISC) {
         dst[3 * NT] = P2{gn[0], gn[1]};
-        dst[4 * NT] = P2{gn[2], gn[3]};
+        dst[4 * NT].a = gn[2];
       }
     } else {
       T* dst = mine1 + slot * (2 * NP * NT);
@@ -489,22 +515,22 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       if (VISC) {
         dst[5 * NT] = W[5];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) dst[(6 + c) * NT] = gn[c];
+        for (int c = 0; c < 3; ++c) dst[(6 + c) * NT] = gn[c];
       }
     }
   };
-  T raw[5], gn[4] = {T(0), T(0), T(0), T(0)};
+  T raw[5], gn[3] = {T(0), T(0), T(0)};
   // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots 0..4.
   // All loads are issued before the first conversion so that their latencies overlap.
   {
-    T raws[YZ_RING][5], gns[YZ_RING][4];
+    T raws[YZ_RING][5], gns[YZ_RING][3];
 #pragma unroll
     for (int s = 0; s < YZ_RING; ++s) {
       const unsigned o = col + (unsigned)(c0 + s) * sm;
 #pragma unroll
       for (int q = 0; q < 5; ++q) raws[s][q] = (U + q * P.vol)[o];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) gns[s][c] = VISC ? gsrc[c][o] : T(0);
+      for (int c = 0; c < 3; ++c) gns[s][c] = VISC ? gsrc[c][o] : T(0);
     }
 #pragma unroll
     for (int s = 0; s < YZ_RING; ++s) put(s, raws[s], gns[s]);
@@ -550,7 +576,7 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       for (int q = 0; q < 5; ++q) raw[q] = (U + q * P.vol)[on];
       if (VISC) {
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) gn[cc] = gsrc[cc][on];
+        for (int cc = 0; cc < 3; ++cc) gn[cc] = gsrc[cc][on];
       }
     }
     if (upd) {
@@ -732,7 +758,10 @@ __global__ void face_flux_kernel(Gas<T> gas, const T* W, const T* Gt, const T* i
   const T* Gf = Gt + (size_t)f * 16;
   auto w0 = [&](int m, int q) -> T { return Wf[(m + 2) * 6 + q]; };   // offsets about cell i
   auto w1 = [&](int m, int q) -> T { return Wf[(m + 3) * 6 + q]; };   // offsets about cell i+1
-  auto g1 = [&](int m, int c) -> T { return Gf[(m + 2) * 4 + c]; };   // offsets about cell i+1
+  auto g1 = [&](int m, int c) -> T {                                    // offsets about cell i+1; the ABI's four
+    const T* r = Gf + (m + 2) * 4;                                       // components -> the three the sweeps carry
+    return c == 0 ? r[0] : c == 1 ? r[2] : r[1] + r[3];
+  };
   T WmL[5], WpL[5], WmR[5], WpR[5];
   weno_cell_states<T, DIR>(w0, WmL, WpL);
   weno_cell_states<T, DIR>(w1, WmR, WpR);

@@ -232,7 +232,8 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
 // from Fr = [mass, n, t1, t2, energy].
 //   w(m, q): primitive q in {rho,u,v,w,p,T} of the cell at offset m in -2..1 along DIR
 //   g(m, c): transverse centre derivatives at offset m in -2..1:
-//            c = 0: d_t1 u_n, 1: d_t1 u_t1, 2: d_t2 u_n, 3: d_t2 u_t2
+//            c = 0: d_t1 u_n, 1: d_t2 u_n, 2: d_t1 u_t1 + d_t2 u_t2 (tau_nn needs only the sum, and the
+//            face interpolation is linear, so the gradient pass stores the sum: 3 arrays per sweep, not 4)
 //   i24Xf: 1/(24 X_xi^f) of this face.   (n,t1,t2) = (DIR, DIR+1, DIR+2) mod 3.
 template <class T, int DIR, class WAcc, class GAcc>
 __device__ __forceinline__ void viscous_sub(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T Fr[5]) {
@@ -248,16 +249,16 @@ __device__ __forceinline__ void viscous_sub(const Gas<T>& gas, const WAcc& w, co
     dn[c] = Num<T>::fma_(T(27), p1 - c0, m1 - p2);
     fv[c] = Num<T>::fma_(T(9), c0 + p1, -(m1 + p2));
   }
-  T gt[4];
+  T gt[3];
 #pragma unroll
-  for (int c = 0; c < 4; ++c)
+  for (int c = 0; c < 3; ++c)
     gt[c] = Num<T>::fma_(T(9), g(-1, c) + g(0, c), -(g(-2, c) + g(1, c)));
   T mu = gas.sutherland ? viscosity<T>(gas, fv[3] * T(1.0 / 16.0)) : gas.mu_ref;
   T mX = mu * i24Xf, mG = mu * T(1.0 / 16.0);
   // tau_nn = mu (2 d_n u_n - 2/3 div) = mu (4/3 d_n u_n - 2/3 (d_t1 u_t1 + d_t2 u_t2))
-  T tnn = Num<T>::fma_(mX * Num<T>::template K<K_4_3>(), dn[0], -(mG * Num<T>::template K<K_2_3>()) * (gt[1] + gt[3]));
+  T tnn = Num<T>::fma_(mX * Num<T>::template K<K_4_3>(), dn[0], -(mG * Num<T>::template K<K_2_3>()) * gt[2]);
   T tn1 = Num<T>::fma_(mX, dn[1], mG * gt[0]);
-  T tn2 = Num<T>::fma_(mX, dn[2], mG * gt[2]);
+  T tn2 = Num<T>::fma_(mX, dn[2], mG * gt[1]);
   Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
   T work = Num<T>::fma_(fv[2], tn2, Num<T>::fma_(fv[1], tn1, fv[0] * tnn));
   Fr[4] = Num<T>::fma_(-(mX * gas.lam_fac), dn[3], Num<T>::fma_(T(-1.0 / 16.0), work, Fr[4]));
