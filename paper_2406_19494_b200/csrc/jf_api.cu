@@ -289,9 +289,27 @@ jf_status launch_halo_axis(jf_solver* s, Impl<T>& I, T* U, int axis) {
   return JF_OK;
 }
 
+// all three passes: one fused launch (halo_all_kernel), or the per-axis passes when a face is JF_BC_EXCHANGE
+// (those are driven pass by pass with the face transfers in between)
 template <class T>
 jf_status launch_halo(jf_solver* s, Impl<T>& I, T* U) {
   jf_status st;
+  bool exchange = false;
+  for (int f = 0; f < 6; ++f) exchange = exchange || I.bc[f].type == 5;
+#ifdef JF_HALO_PER_AXIS
+  exchange = true;
+#endif
+  if (!exchange) {
+    const jf::Params<T>& P = I.P;
+    const long long tot = 6LL * ((long long)P.n[1] * P.n[2] + (long long)P.P[0] * P.n[2] + (long long)P.P[0] * P.P[1]);
+    jf::HaloFaces<T> B;
+    for (int f = 0; f < 6; ++f) B.f[f] = I.bc[f];
+    Timed t(s, K_HALO);
+    jf::halo_all_kernel<T><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(P, B, U);
+    s->launches += 1;
+    JF_CUDA(s, cudaPeekAtLastError());
+    return JF_OK;
+  }
   for (int a = 0; a < 3; ++a)
     if ((st = launch_halo_axis<T>(s, I, U, a))) return st;
   return JF_OK;

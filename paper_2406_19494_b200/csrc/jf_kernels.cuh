@@ -42,36 +42,24 @@ struct FaceBC {
 };
 
 // ------------------------------------------------------------------ a1 halo fill
-// One launch per axis, both sides, 3 layers.  AXIS 0: (j,k) interior; AXIS 1: all padded i, k
-// interior; AXIS 2: all padded (i,j).  Thread -> (p1 fastest, p2, side*3+m-1).
+// The boundary pass of one axis assigns every ghost cell from ONE source cell of the same tangential position
+// (periodic image, nearest interior cell, mirror cell; none for a Dirichlet face), so the x -> y -> z order of
+// reading O3 is a composition of per-cell maps.  bc_src gives the source index of a pass, bc_ghost its map on the
+// conservative state; halo_kernel<AXIS> applies one pass, halo_all_kernel composes the three per ghost cell.
+__device__ __forceinline__ int bc_src(int type, int side, int m, int N) {
+  if (type == 0) return (side == 0 ? N - m : m - 1) + NH;          // periodic image
+  if (type == 1) return (side == 0 ? 0 : N - 1) + NH;              // zero gradient: nearest interior cell
+  return (side == 0 ? m - 1 : N - m) + NH;                         // wall: mirror cell (Dirichlet: unused)
+}
+
+// Ghost state of the pass along AXIS on face `f` (side 0 / 1) at padded tangential indices (p1, p2), from the
+// conservative state Us of the pass's source cell.  Periodic / zero-gradient: a copy.
 template <class T, int AXIS>
-__global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, FaceBC<T> bhi, T* U) {
+__device__ __forceinline__ void bc_ghost(const Params<T>& P, const FaceBC<T>& f, int p1, int p2, const T Us[5], T Ug[5]) {
   constexpr int t1a = (AXIS == 0) ? 1 : 0, t2a = (AXIS == 2) ? 1 : 2;
-  const int lo1 = (AXIS == 0) ? NH : 0, n1 = (AXIS == 0) ? P.n[1] : P.P[0];
-  const int lo2 = (AXIS == 2) ? 0 : NH, n2 = (AXIS == 2) ? P.P[1] : P.n[2];
-  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  long long total = (long long)n1 * n2 * 6;
-  if (tid >= total) return;
-  int a1, a2, sm;
-  if (AXIS == 0) {              // x ghosts: make (side,m) fastest so neighbouring threads touch one line
-    sm = (int)(tid % 6); a1 = (int)((tid / 6) % n1); a2 = (int)(tid / (6LL * n1));
-  } else {
-    a1 = (int)(tid % n1); a2 = (int)((tid / n1) % n2); sm = (int)(tid / ((long long)n1 * n2));
-  }
-  const int side = sm / 3, m = sm % 3 + 1;
-  const int p1 = lo1 + a1, p2 = lo2 + a2;
-  const FaceBC<T>& f = side ? bhi : blo;
-  const int N = P.n[AXIS];
-  const int g = (side == 0 ? -m : N - 1 + m) + NH;
-  long long str[3] = {1, P.sy, P.sz};
-  long long tang = (long long)p1 * str[t1a] + (long long)p2 * str[t2a];
-  long long og = tang + (long long)g * str[AXIS];
-  if (f.type == 5) return;      // JF_BC_EXCHANGE: filled from the neighbouring block (face_xfer_kernel)
   if (f.type == 0 || f.type == 1) {
-    int src = f.type == 0 ? (side == 0 ? N - m : m - 1) : (side == 0 ? 0 : N - 1);
-    long long os = tang + (long long)(src + NH) * str[AXIS];
 #pragma unroll
-    for (int q = 0; q < 5; ++q) U[q * P.vol + og] = U[q * P.vol + os];
+    for (int q = 0; q < 5; ++q) Ug[q] = Us[q];
     return;
   }
   const Gas<T>& gas = P.gas;
@@ -82,10 +70,8 @@ __global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, F
 #pragma unroll
     for (int q = 0; q < 5; ++q) W[q] = T(f.dirichlet[((long long)q * m2 + c2) * m1 + c1]);
   } else {
-    int r = (side == 0 ? m - 1 : N - m) + NH;
-    long long orr = tang + (long long)r * str[AXIS];
     T Wr[6];
-    cons_to_prim<T>(gas, U[orr], U[P.vol + orr], U[2 * P.vol + orr], U[3 * P.vol + orr], U[4 * P.vol + orr], Wr);
+    cons_to_prim<T>(gas, Us[0], Us[1], Us[2], Us[3], Us[4], Wr);
     // exact division for T_r as the definition states it (ghost density depends on it)
     T Tr = Wr[4] / (Wr[0] * gas.Rgas);
     T uw[3] = {f.uw[0], f.uw[1], f.uw[2]};
@@ -111,11 +97,118 @@ __global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, F
     W[4] = Wr[4];
     W[0] = Wr[4] / (gas.Rgas * Tg);
   }
-  U[og] = W[0];
-  U[P.vol + og] = W[0] * W[1];
-  U[2 * P.vol + og] = W[0] * W[2];
-  U[3 * P.vol + og] = W[0] * W[3];
-  U[4 * P.vol + og] = W[4] / gas.gm1 + T(0.5) * W[0] * (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+  Ug[0] = W[0];
+  Ug[1] = W[0] * W[1];
+  Ug[2] = W[0] * W[2];
+  Ug[3] = W[0] * W[3];
+  Ug[4] = W[4] / gas.gm1 + T(0.5) * W[0] * (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+}
+
+// One launch per axis, both sides, 3 layers.  AXIS 0: (j,k) interior; AXIS 1: all padded i, k
+// interior; AXIS 2: all padded (i,j).  Thread -> (p1 fastest, p2, side*3+m-1).
+template <class T, int AXIS>
+__global__ void __launch_bounds__(256) halo_kernel(Params<T> P, FaceBC<T> blo, FaceBC<T> bhi, T* U) {
+  constexpr int t1a = (AXIS == 0) ? 1 : 0, t2a = (AXIS == 2) ? 1 : 2;
+  const int lo1 = (AXIS == 0) ? NH : 0, n1 = (AXIS == 0) ? P.n[1] : P.P[0];
+  const int lo2 = (AXIS == 2) ? 0 : NH, n2 = (AXIS == 2) ? P.P[1] : P.n[2];
+  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long total = (long long)n1 * n2 * 6;
+  if (tid >= total) return;
+  int a1, a2, sm;
+  if (AXIS == 0) {              // x ghosts: make (side,m) fastest so neighbouring threads touch one line
+    sm = (int)(tid % 6); a1 = (int)((tid / 6) % n1); a2 = (int)(tid / (6LL * n1));
+  } else {
+    a1 = (int)(tid % n1); a2 = (int)((tid / n1) % n2); sm = (int)(tid / ((long long)n1 * n2));
+  }
+  const int side = sm / 3, m = sm % 3 + 1;
+  const int p1 = lo1 + a1, p2 = lo2 + a2;
+  const FaceBC<T>& f = side ? bhi : blo;
+  const int N = P.n[AXIS];
+  const int g = (side == 0 ? -m : N - 1 + m) + NH;
+  long long str[3] = {1, P.sy, P.sz};
+  long long tang = (long long)p1 * str[t1a] + (long long)p2 * str[t2a];
+  long long og = tang + (long long)g * str[AXIS];
+  if (f.type == 5) return;      // JF_BC_EXCHANGE: filled from the neighbouring block (face_xfer_kernel)
+  const long long os = tang + (long long)bc_src(f.type, side, m, N) * str[AXIS];
+  T Us[5], Ug[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Us[q] = (f.type == 2) ? T(1) : U[q * P.vol + os];
+  bc_ghost<T, AXIS>(P, f, p1, p2, Us, Ug);
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U[q * P.vol + og] = Ug[q];
+}
+
+// The three passes in one launch (no JF_BC_EXCHANGE face): one thread per ghost cell.  The cell's chain of
+// sources is followed backwards (z, then y, then x) to an interior cell, whose state is then mapped forwards
+// through the passes that own the cell's ghost indices (x, then y, then z) - the value the three launches of
+// halo_kernel leave in that cell, from the same instruction sequences (`keep` stops the compiler from
+// contracting across the stages, which are separated by a store and a load in the per-axis passes).
+// Reads interior cells only, writes ghost cells only.  Thread order: x slabs ((side,m) fastest, interior j,k),
+// then y slabs (all padded i, interior k), then z slabs (all padded i,j).
+__device__ __forceinline__ void keep(double& x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void keep(float& x) { asm volatile("" : "+f"(x)); }
+__device__ __forceinline__ void keep(Dual& x) { asm volatile("" : "+d"(x.v), "+d"(x.d)); }
+
+template <class T>
+struct HaloFaces { FaceBC<T> f[6]; };
+
+template <class T>
+__global__ void __launch_bounds__(256) halo_all_kernel(Params<T> P, HaloFaces<T> B, T* U) {
+  const int nx = P.n[0], ny = P.n[1], nz = P.n[2], Px = P.P[0], Py = P.P[1];
+  const long long cx = 6LL * ny * nz, cy = 6LL * Px * nz, cz = 6LL * Px * Py;
+  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int pi, pj, pk;
+  if (tid < cx) {
+    const int sm = (int)(tid % 6), side = sm / 3, m = sm % 3 + 1;
+    pi = (side == 0 ? -m : nx - 1 + m) + NH;
+    pj = (int)((tid / 6) % ny) + NH; pk = (int)(tid / (6LL * ny)) + NH;
+  } else if (tid < cx + cy) {
+    tid -= cx;
+    pi = (int)(tid % Px);
+    const int sm = (int)((tid / Px) % 6), side = sm / 3, m = sm % 3 + 1;
+    pj = (side == 0 ? -m : ny - 1 + m) + NH;
+    pk = (int)(tid / (6LL * Px)) + NH;
+  } else if (tid < cx + cy + cz) {
+    tid -= cx + cy;
+    pi = (int)(tid % Px); pj = (int)((tid / Px) % Py);
+    const int sm = (int)(tid / ((long long)Px * Py)), side = sm / 3, m = sm % 3 + 1;
+    pk = (side == 0 ? -m : nz - 1 + m) + NH;
+  } else {
+    return;
+  }
+  // ghost layer of an index: side 0 / 1 and m = 1..3, or m = 0 for an interior index
+  auto layer = [](int p, int n, int& side) -> int {
+    if (p < NH) { side = 0; return NH - p; }
+    if (p >= n + NH) { side = 1; return p - (n + NH) + 1; }
+    side = 0; return 0;
+  };
+  int sdx, sdy, sdz;
+  const int mx = layer(pi, nx, sdx), my = layer(pj, ny, sdy), mz = layer(pk, nz, sdz);
+  const int si = mx ? bc_src(B.f[sdx].type, sdx, mx, nx) : pi;
+  const int sj = my ? bc_src(B.f[2 + sdy].type, sdy, my, ny) : pj;
+  const int sk = mz ? bc_src(B.f[4 + sdz].type, sdz, mz, nz) : pk;
+  const long long os = (long long)sk * P.sz + (long long)sj * P.sy + si;
+  T Ua[5], Ub[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Ua[q] = U[q * P.vol + os];
+  if (mx) {
+    bc_ghost<T, 0>(P, B.f[sdx], sj, sk, Ua, Ub);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Ua[q] = Ub[q]; keep(Ua[q]); }
+  }
+  if (my) {
+    bc_ghost<T, 1>(P, B.f[2 + sdy], pi, sk, Ua, Ub);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Ua[q] = Ub[q]; keep(Ua[q]); }
+  }
+  if (mz) {
+    bc_ghost<T, 2>(P, B.f[4 + sdz], pi, pj, Ua, Ub);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) Ua[q] = Ub[q];
+  }
+  const long long og = (long long)pk * P.sz + (long long)pj * P.sy + pi;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U[q * P.vol + og] = Ua[q];
 }
 
 // ------------------------------------------------------------------ a1 across blocks: face transfer

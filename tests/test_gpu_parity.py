@@ -95,6 +95,35 @@ def test_halo_fill_every_cell(jf, ora, which, dtype):
         assert np.array_equal(Ug, Uo)                         # pure copies are bit-exact
 
 
+@pytest.mark.parametrize("which", [-1, 0, 1, 2, 3])
+@pytest.mark.parametrize("dtype", ["f64", "f32", "f64t"])
+def test_fused_halo_launch_equals_the_three_axis_passes_bitwise(jf, which, dtype):
+    # jf_fill_halo is ONE launch that composes the x -> y -> z passes per ghost cell (reading O3);
+    # jf_fill_halo_axis runs them one by one: same bits in every padded cell, NaN-poisoned halos on entry
+    if which == 3:
+        c = cases.flat_plate(nx=64, ny=24, nz=8)
+    else:
+        c = cases.random_admissible(n=(12, 10, 8), seed=1, stretched=True) if which < 0 else all_bc_case(which=which, n=(37, 21, 13))
+    import torch
+    s = jf.Solver(c, dtype)
+    if dtype == "f64t":
+        s.jf_set_tangent_seed(0.7, -0.3)
+        rng = np.random.default_rng(5)
+        U0 = s.state(dU0=rng.uniform(-0.1, 0.1, np.asarray(c.U0).shape))
+    else:
+        U0 = s.state()
+    poison = torch.full_like(U0, float("nan"))
+    poison[INT] = U0[INT]
+    Ua, Ub = poison.clone(), poison.clone()
+    s.jf_fill_halo(Ua)
+    for axis in range(3):
+        s.jf_fill_halo_axis(Ub.data_ptr(), axis)
+    torch.cuda.synchronize()
+    a, b = Ua.cpu().numpy(), Ub.cpu().numpy()
+    assert np.isfinite(a).all() and np.isfinite(b).all()
+    assert a.tobytes() == b.tobytes()
+
+
 def test_disturbance_A0_is_plain_wall_on_gpu(jf):
     # PAPER.md:104
     bc = cases.periodic_bc()
@@ -399,4 +428,4 @@ def test_abi_error_statuses(jf):
     n0 = s.jf_launch_count()
     s.jf_rk3_step(U, 1e-3)
     torch.cuda.synchronize()
-    assert s.jf_launch_count() - n0 == 3 * (3 + 4)
+    assert s.jf_launch_count() - n0 == 3 * (1 + 4)
