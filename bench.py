@@ -219,7 +219,7 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = solver.jf_launch_count() - l0
     # the same K steps once more with an event pair around every launch (jf_diag_timing): per-kernel durations for
-    # the roofline of the dominant kernel.  Kept out of the region above because the 42 extra event records per
+    # the roofline of the dominant kernel.  Kept out of the region above because the 30 extra event records per
     # step cost 2 % at 256^3 and 10-40 % on the small boxes.
     solver.jf_diag_kernel_times()                      # reset
     solver.jf_diag_timing(True)

@@ -109,7 +109,9 @@ size_t jf_state_elems(const jf_solver *s);
 
 /* Halo / boundary fill (:80, :100-104, Eq. 8), in place, asynchronous.  Order x, y, z; the y
  * pass runs over all padded i and the z pass over all padded (i,j), which defines every edge
- * and corner cell. */
+ * and corner cell.  Without a JF_BC_EXCHANGE face the three passes are ONE launch that composes them
+ * per ghost cell (each pass maps one source cell to one ghost cell); the result is bitwise that of
+ * jf_fill_halo_axis(0), (1), (2). */
 jf_status jf_fill_halo(jf_solver *s, void *U_dev);
 
 /* R = R_NSE(U) of Eq. 6 on interior cells (halo cells of R are left untouched).  The halos of
