@@ -250,8 +250,11 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
 
 // Segment length of the marching (y / z) sweeps.  Each segment costs two extra WENO steps, one extra
 // face and a window prologue, so segments should be long; but the grid must still fill the 148 SMs
-// (12 resident warps each) for several waves.  Largest power-of-two length (<= N) that leaves at
-// least JF_SEG_WAVES waves of warps, never below 8 cells.
+// (12 resident warps each) for several waves.  Small grids: equal segments for about 2.5 waves of warps
+// (measured best on the 192x128x128 channel, 128^3 and 192^3: L = 22, 15, 48; fewer, longer segments
+// leave SMs idle in the last wave, shorter ones pay the per-segment extras), never below 8 cells.  When
+// that length reaches 64 the extras are below 4 % and the old rule is kept: largest power-of-two length
+// (<= N) that leaves at least JF_SEG_WAVES waves (256^3: 64; 37...86 measured within 1 %).
 #ifndef JF_GM_WAVES
 #define JF_GM_WAVES 8
 #endif
@@ -262,7 +265,13 @@ int pick_segment(long long warps_per_layer, int N) {
 #ifdef JF_SEG_FORCE
   return JF_SEG_FORCE < N ? JF_SEG_FORCE : N;
 #endif
-  const long long want = (long long)JF_SEG_WAVES * 148 * 12;
+  const long long cap = 148 * 12;
+  {
+    const long long nseg = (5 * cap / 2 + warps_per_layer - 1) / warps_per_layer;
+    const int Ls = (int)std::max<long long>((N + nseg - 1) / nseg, 8);
+    if (Ls < 64) return Ls < N ? Ls : N;
+  }
+  const long long want = (long long)JF_SEG_WAVES * cap;
   int L = 8;
   while (L < N) L *= 2;                      // one segment
   while (L > 8 && warps_per_layer * ((N + L - 1) / L) < want) L /= 2;
