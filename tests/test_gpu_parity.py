@@ -322,35 +322,46 @@ def test_config4_tgv128_2_steps_fp64_and_fp32(jf, ora):
 
 # ------------------------------------------------------------------ error behaviour of the ABI
 # ------------------------------------------------------------------ full size, sampled (bench.py's launch configuration)
+def _gather(U, idx):
+    """U[:, idx_z][:, :, idx_y][:, :, :, idx_x] of a device state array, as float64 on the host."""
+    import torch
+    iz, iy, ix = (torch.as_tensor(np.asarray(idx[a]), device=U.device) for a in (2, 1, 0))
+    return U.index_select(1, iz).index_select(2, iy).index_select(3, ix).cpu().numpy().astype(np.float64)
+
+
 def _sub_box_case(c, U, lo, m):
-    """Periodic m^3 case cut out of the periodic state U (full padded array) at interior offset lo."""
+    """Periodic m^3 case cut out of the periodic device state U (full padded array) at interior offset lo."""
     idx = [(np.arange(m) + lo[a]) % c.n[a] + NH for a in range(3)]
     sub = cases.empty_state((m, m, m))
-    sub[(slice(None),) + (slice(NH, -NH),) * 3] = U[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+    sub[(slice(None),) + (slice(NH, -NH),) * 3] = _gather(U, idx)
     dx = c.xf[1] - c.xf[0]
     f = cases.uniform_faces(0.0, m * dx, m)
     return cases.Case(name="sub", n=(m, m, m), xf=f, yf=f.copy(), zf=f.copy(), gamma=c.gamma, R_gas=c.R_gas,
                       Pr=c.Pr, mu=c.mu, bc=cases.periodic_bc(), U0=sub, dt=c.dt, n_steps=1)
 
 
-@pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_config4_tgv256_sampled_against_oracle_sub_boxes(jf, ora, dtype):
-    """256^3 (the size bench.py times, same kernels / grids / segment lengths): two RK3 steps on the GPU,
-    then the second step is checked on sampled 16^3 blocks.  One RK3 step moves information by at most
-    3 stages x 3 cells, so the oracle stepping a periodic 40^3 cut-out of the GPU's own step-1 state is
-    exact on the central 16^3 (margin 12 >= 9) whatever its (wrong) periodic wrap does at the rim."""
-    c = cases.tgv(256)
+@pytest.mark.parametrize("n,dtype", [(256, "f64"), (256, "f32"), (384, "f64"), (512, "f64"), (512, "f32")])
+def test_config4_full_size_sampled_against_oracle_sub_boxes(jf, ora, n, dtype):
+    """256^3 (the size bench.py times), 384^3 fp64 and 512^3 fp64 / fp32 (the largest lines of configs[4]), same
+    kernels / grids / segment lengths as bench.py launches: two RK3 steps on the GPU, then the second step
+    is checked on sampled 16^3 blocks.  One RK3 step moves information by at most 3 stages x 3 cells, so the
+    oracle stepping a periodic 40^3 cut-out of the GPU's own step-1 state is exact on the central 16^3
+    (margin 12 >= 9) whatever its (wrong) periodic wrap does at the rim.  Cut-outs are gathered on the device."""
+    import torch
+    c = cases.tgv(n)
     s = jf.Solver(c, dtype)
     U = s.state()
     s.jf_rk3_step(U, c.dt)
-    U1 = U.cpu().numpy().astype(np.float64)
+    U1 = U.clone()
     s.jf_rk3_step(U, c.dt)
-    U2 = U.cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
     m, g = 40, 12
     rng = np.random.default_rng(11)
-    los = [(0, 0, 0), (250, 3, 121), (100, 250, 250)] + [tuple(int(v) for v in rng.integers(0, 256, 3)) for _ in range(3)]
-    mom = np.max(np.sqrt(U2[1] ** 2 + U2[2] ** 2 + U2[3] ** 2))
-    scale = [np.max(np.abs(U2[0])), mom, mom, mom, np.max(np.abs(U2[4]))]
+    los = [(0, 0, 0), (n - 6, 3, n // 2 - 7), (100, n - 6, n - 6)] + [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(3)]
+    Ud = U.double()
+    mom = float(torch.sqrt(Ud[1] ** 2 + Ud[2] ** 2 + Ud[3] ** 2).max())
+    scale = [float(Ud[0].abs().max()), mom, mom, mom, float(Ud[4].abs().max())]
+    del Ud
     worst = np.zeros(5)
     for lo in los:
         sc = _sub_box_case(c, U1, lo, m)
@@ -358,12 +369,12 @@ def test_config4_tgv256_sampled_against_oracle_sub_boxes(jf, ora, dtype):
         Uo = o.state()
         o.rk3_step(Uo, c.dt)
         Uo = np.asarray(Uo, dtype=np.float64)
-        idx = [(np.arange(g, m - g) + lo[a]) % 256 + NH for a in range(3)]
-        got = U2[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+        idx = [(np.arange(g, m - g) + lo[a]) % n + NH for a in range(3)]
+        got = _gather(U, idx)
         ref = Uo[:, NH + g:NH + m - g, NH + g:NH + m - g, NH + g:NH + m - g]
         for q in range(5):
             worst[q] = max(worst[q], np.max(np.abs(got[q] - ref[q])) / scale[q])
-    print("tgv256", dtype, "sampled parity", worst)
+    print(f"tgv{n}", dtype, "sampled parity", worst)
     assert np.all(worst <= TOL[dtype]), worst
 
 
