@@ -86,6 +86,13 @@ typedef struct {
   double nb_width[3];      /* JF_BC_EXCHANGE: widths of the neighbouring block's three cells next to
                               this face, nearest first (> 0): the halo cells then carry the geometry
                               they have on the undivided grid (stretched axes included)              */
+  int nb_has_face;         /* JF_BC_EXCHANGE across an interior cut (not a periodic wrap): nb_face holds  */
+  double nb_face[3];       /* the coordinates of the neighbour's three faces beyond this one, nearest
+                              first; widths and centres of the halo cells are then formed from them as
+                              for interior cells (xf[i+1]-xf[i], (xf[i]+xf[i+1])/2: the undivided grid's
+                              values bit for bit) and nb_width is ignored.  Across a periodic wrap
+                              (nb_has_face = 0) the undivided grid itself copies widths and accumulates
+                              centres outward, which is what nb_width reproduces                      */
 } jf_bc_face;
 typedef struct { jf_bc_face face[6]; } jf_bc; /* x-, x+, y-, y+, z-, z+; periodic must pair */
 
@@ -205,7 +212,7 @@ jf_status jf_diag_alu_peak(jf_dtype dtype, int iters, double *flops_host, double
 /* Per-kernel device timing (diagnostic).  jf_diag_timing(s, 1) makes every launch of this solver
  * record a CUDA-event pair on its stream; jf_diag_kernel_times synchronises the stream, writes the
  * accumulated milliseconds and launch counts per kernel class since the previous call (6 classes:
- * 0 halo (3 launches per fill), 1 gradient, 2 x sweep, 3 y sweep, 4 z sweep + RK3 stage, 5 CFL)
+ * 0 halo (one fused launch per fill; three per-axis passes for decomposed blocks), 1 gradient, 2 x sweep, 3 y sweep, 4 z sweep + RK3 stage, 5 CFL)
  * and resets them.  jf_diag_kernel_name(k) names class k ("" if out of range). */
 jf_status jf_diag_timing(jf_solver *s, int enable);
 jf_status jf_diag_kernel_times(jf_solver *s, double ms[6], unsigned long long launches[6]);
@@ -220,6 +227,15 @@ const char *jf_diag_kernel_name(int k);
 jf_status jf_diag_face_flux(jf_dtype dtype, int dir, double gamma, double R_gas, double Pr,
                             const jf_mu_law *mu, int n_faces, const double *W, const double *Gt,
                             const double *Xf, double *F);
+
+/* Geometry tables the kernels read, copied back from the workspace (diagnostic; synchronises): for axis
+ * a in 0..2, HOST arrays of n_a + 6 doubles (padded index p = i + 3; any pointer may be NULL):
+ *   inv_delta[p] = 1/Delta_p,  centre[p] = cell centre,  i12Xc[p] = 1/(12 X_xi^c) (interior p only, else 1/12),
+ *   i24Xf[p] = 1/(24 X_xi^f) of the face on the high side of cell p (p = 2 .. n+2, else 1/24)
+ * (reading O2; halo geometry: periodic copy, mirror, or the neighbour widths of a JF_BC_EXCHANGE
+ * face).  Values are those of the solver dtype converted to double.  tests/test_gpu_units.py compares them with
+ * the oracle's own tables. */
+jf_status jf_diag_metrics(jf_solver *s, int axis, double *inv_delta, double *centre, double *i12Xc, double *i24Xf);
 
 /* Library version / build info string (static storage). */
 const char *jf_version(void);

@@ -12,7 +12,8 @@
  *
  * Layout (Nh = 3): U[5][nz+6][ny+6][nx+6], x fastest,
  *   index ((q*(nz+6)+k+3)*(ny+6)+j+3)*(nx+6)+i+3, q in {rho, rho*u, rho*v, rho*w, E}.
- * All pointers are HOST pointers.  dtype 0 = double, 1 = float.
+ * All pointers are HOST pointers.  dtype 0 = double, 1 = float, 2 = long double (the arbiter:
+ * same text instantiated on a 64-bit mantissa, rational constants formed in that precision).
  */
 #ifndef ORA_H
 #define ORA_H
@@ -24,7 +25,8 @@ extern "C" {
 typedef struct ora_solver ora_solver;
 
 enum { ORA_OK = 0, ORA_EINVAL = 1, ORA_ENOTFINITE = 5 };
-enum { ORA_F64 = 0, ORA_F32 = 1 };
+enum { ORA_F64 = 0, ORA_F32 = 1,
+       ORA_F80 = 2 /* x87 long double (16-byte elements): the arbiter instantiation, tests only */ };
 enum { ORA_BC_PERIODIC = 0, ORA_BC_ZEROGRAD = 1, ORA_BC_DIRICHLET = 2,
        ORA_BC_WALL_ISOTHERMAL = 3, ORA_BC_WALL_ADIABATIC = 4 };
 
@@ -77,6 +79,9 @@ int ora_count_flops_part(ora_solver *s, const void *U, int what, double counts[4
 
 /* grid metrics (padded arrays of length n+6 for axis a in 0..2): widths and centres */
 int ora_metrics(const ora_solver *s, int axis, double *delta, double *centre);
+/* index-space metrics of O2: Xc[p] = X_xi^c at padded cell p (interior p; 0 elsewhere), Xf[p] = X_xi^f of
+   the face on the high side of padded cell p (p = 2 .. n+2; 0 elsewhere) */
+int ora_metrics_index(const ora_solver *s, int axis, double *Xc, double *Xf);
 
 /* --- unit-level functions for the pins (double) --- */
 /* WENO5-JS value at the face between v[2] and v[3], stencil v[0..4] */

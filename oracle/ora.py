@@ -48,7 +48,8 @@ _libs = {}
 
 def lib(variant="ref"):
     """variant "ref": the oracle (-ffp-contract=off).  "fma": same sources with FMA contraction,
-    only for measuring the oracle's own round-off sensitivity."""
+    only for measuring the oracle's own round-off sensitivity.  "asan": same sources under
+    AddressSanitizer + UBSan (needs libasan preloaded: tests/test_oracle_sanitizers.py)."""
     if variant not in _libs:
         path = _build.build(variant=variant)
         L = C.CDLL(path)
@@ -69,6 +70,7 @@ def lib(variant="ref"):
         L.ora_count_flops_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double, c_double_p]
         L.ora_count_flops_part.argtypes = [C.c_void_p, C.c_void_p, C.c_int, c_double_p]
         L.ora_metrics.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p]
+        L.ora_metrics_index.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p]
         L.ora_weno5.argtypes = [c_double_p]
         L.ora_weno5.restype = C.c_double
         L.ora_weno5_detail.argtypes = [c_double_p] * 4
@@ -111,7 +113,9 @@ class Oracle:
     def __init__(self, case, dtype="f64", variant="ref"):
         self.case = case
         self.L = lib(variant)
-        self.np_dtype = np.float64 if dtype == "f64" else np.float32
+        self.np_dtype = {"f64": np.float64, "f32": np.float32, "f80": np.longdouble}[dtype]
+        if dtype == "f80":
+            assert np.finfo(np.longdouble).nmant == 63 and np.dtype(np.longdouble).itemsize == 16
         self._keep = []
         nx, ny, nz = case.n
         xf, yf, zf = _arr(case.xf, nx + 1), _arr(case.yf, ny + 1), _arr(case.zf, nz + 1)
@@ -133,7 +137,7 @@ class Oracle:
                 b.dist = Disturbance(1, fb.dist["A"], fb.dist["kappa"], fb.dist["t1_lo"], fb.dist["t1_hi"])
         ga = _arr(case.body_accel, 3)
         h = C.c_void_p()
-        st = self.L.ora_create(C.byref(h), C.byref(g), 0 if dtype == "f64" else 1, case.gamma, case.R_gas,
+        st = self.L.ora_create(C.byref(h), C.byref(g), {"f64": 0, "f32": 1, "f80": 2}[dtype], case.gamma, case.R_gas,
                               case.Pr, C.byref(mu), C.byref(bc), _dp(ga))
         if st != 0:
             raise ValueError(f"ora_create failed with status {st}")
@@ -199,6 +203,12 @@ class Oracle:
         assert self.L.ora_metrics(self.h, axis, _dp(d), _dp(c)) == 0
         return d, c
 
+    def metrics_index(self, axis):
+        n = self.case.n[axis] + 6
+        Xc, Xf = np.zeros(n), np.zeros(n)
+        assert self.L.ora_metrics_index(self.h, axis, _dp(Xc), _dp(Xf)) == 0
+        return Xc, Xf
+
     def viscous_face(self, U, d, i, j, k):
         self._chk(U)
         F = np.zeros(5)
@@ -206,10 +216,19 @@ class Oracle:
         return F
 
 
-def run_case(case, dtype="f64", n_steps=None, log=None, variant="ref"):
+def run_case(case, dtype="f64", n_steps=None, log=None, variant="ref", dts_in=None):
     """Advance a case with the oracle exactly as the drivers do: fixed dt x n_steps, or CFL steps
-    (clipped to t_end when given).  Returns (U, list of dt)."""
+    (clipped to t_end when given).  Returns (U, list of dt).  dts_in: take these time steps instead
+    (the arbiter run "f80" is fed the fp64 oracle's own sequence, so that the two differ by the
+    rounding of the scheme's arithmetic only)."""
     o = Oracle(case, dtype, variant)
+    if dts_in is not None:
+        U = o.state()
+        for step, dt in enumerate(dts_in):
+            o.rk3_step(U, dt)
+            if log:
+                log(step + 1, None, dt)
+        return U, list(dts_in)
     U = o.state()
     dts, t = [], 0.0
     n = n_steps if n_steps is not None else case.n_steps

@@ -24,7 +24,7 @@ int ora_create(ora_solver** out, const ora_grid* g, int dtype, double gamma, dou
   if (!g || !mu || !bc) return ORA_EINVAL;
   if (g->nx < 4 || g->ny < 4 || g->nz < 4 || !g->xf || !g->yf || !g->zf) return ORA_EINVAL;
   if (!(gamma > 1.0) || !(Pr > 0.0) || !(mu->mu_ref >= 0.0) || !(R_gas > 0.0)) return ORA_EINVAL;
-  if (dtype != ORA_F64 && dtype != ORA_F32) return ORA_EINVAL;
+  if (dtype != ORA_F64 && dtype != ORA_F32 && dtype != ORA_F80) return ORA_EINVAL;
   const double* xf[3] = {g->xf, g->yf, g->zf};
   int n[3] = {g->nx, g->ny, g->nz};
   for (int a = 0; a < 3; ++a)
@@ -69,6 +69,7 @@ size_t ora_state_elems(const ora_solver* s) { return (size_t)5 * s->c.P[0] * s->
 int ora_fill_halo(ora_solver* s, void* U) {
   if (!s || !U) return ORA_EINVAL;
   if (s->dtype == ORA_F64) ora::fill_halo<double>(s->c, (double*)U);
+  else if (s->dtype == ORA_F80) ora::fill_halo<long double>(s->c, (long double*)U);
   else ora::fill_halo<float>(s->c, (float*)U);
   return ORA_OK;
 }
@@ -76,6 +77,7 @@ int ora_fill_halo(ora_solver* s, void* U) {
 int ora_rhs(ora_solver* s, const void* U, void* R) {
   if (!s || !U || !R) return ORA_EINVAL;
   if (s->dtype == ORA_F64) ora::rhs<double>(s->c, (const double*)U, (double*)R, true, true, true);
+  else if (s->dtype == ORA_F80) ora::rhs<long double>(s->c, (const long double*)U, (long double*)R, true, true, true);
   else ora::rhs<float>(s->c, (const float*)U, (float*)R, true, true, true);
   return ORA_OK;
 }
@@ -95,6 +97,7 @@ int ora_rhs_naive(ora_solver* s, const void* U, void* R) {
 int ora_rk3_step(ora_solver* s, void* U, double dt) {
   if (!s || !U) return ORA_EINVAL;
   if (s->dtype == ORA_F64) ora::rk3_step<double>(s->c, (double*)U, dt);
+  else if (s->dtype == ORA_F80) ora::rk3_step<long double>(s->c, (long double*)U, (long double)dt);
   else ora::rk3_step<float>(s->c, (float*)U, (float)dt);
   return ORA_OK;
 }
@@ -102,6 +105,7 @@ int ora_rk3_step(ora_solver* s, void* U, double dt) {
 int ora_cfl_dt(ora_solver* s, const void* U, double cfl, double* dt) {
   if (!s || !U || !dt) return ORA_EINVAL;
   if (s->dtype == ORA_F64) return ora::cfl_dt<double>(s->c, (const double*)U, cfl, dt);
+  if (s->dtype == ORA_F80) return ora::cfl_dt<long double>(s->c, (const long double*)U, cfl, dt);
   return ora::cfl_dt<float>(s->c, (const float*)U, cfl, dt);
 }
 
@@ -162,6 +166,15 @@ int ora_metrics(const ora_solver* s, int axis, double* delta, double* centre) {
   for (int p = 0; p < s->c.P[axis]; ++p) {
     if (delta) delta[p] = s->c.dl[axis][p];
     if (centre) centre[p] = s->c.xc[axis][p];
+  }
+  return ORA_OK;
+}
+
+int ora_metrics_index(const ora_solver* s, int axis, double* Xc, double* Xf) {
+  if (!s || axis < 0 || axis > 2) return ORA_EINVAL;
+  for (int p = 0; p < s->c.P[axis]; ++p) {
+    if (Xc) Xc[p] = s->c.Xc[axis][p];
+    if (Xf) Xf[p] = s->c.Xf[axis][p];
   }
   return ORA_OK;
 }

@@ -19,6 +19,20 @@ inline double s_abs(double a) { return std::fabs(a); }
 inline float  s_abs(float a)  { return std::fabs(a); }
 inline double s_val(double a) { return a; }
 inline double s_val(float a)  { return (double)a; }
+// Extended precision (x87 long double, 64-bit mantissa): the ARBITER instantiation.  It gives the
+// discrete scheme's own result ~2000 times more accurately than double, so that "GPU vs oracle"
+// differences at the 1e-10 level can be judged by who is closer to it (tests/test_gpu_parity.py).
+inline long double s_sqrt(long double a) { return std::sqrt(a); }
+inline long double s_min(long double a, long double b) { return a < b ? a : b; }
+inline long double s_max(long double a, long double b) { return a > b ? a : b; }
+inline long double s_abs(long double a) { return std::fabs(a); }
+inline double s_val(long double a) { return (double)a; }
+
+// Rational constants num/den of the scheme (13/12, 1/6, 1/10, 2/3, eps = 1/10^6, ...).  double, float
+// and the counting type take the double-rounded quotient exactly as before this helper existed;
+// the arbiter forms the quotient in its own precision (a double-rounded 0.1 would cap it at 1e-17).
+template <class R> inline R cst(double num, double den) { return R(num / den); }
+template <> inline long double cst<long double>(double num, double den) { return (long double)num / (long double)den; }
 
 // Flop-counting scalar: add/sub/mul/min/max = 1, div = 1, sqrt = 1 (each tallied apart);
 // abs / sign / compare / select = 0 (SURVEY §8(d) convention).
@@ -72,7 +86,7 @@ inline R viscosity(int sutherland, R mu_ref, R T_ref, R S, R T) {
 template <class R>
 inline R weno5(R v0, R v1, R v2, R v3, R v4, R* beta_out = nullptr, R* om_out = nullptr,
                R* p_out = nullptr) {
-  const R eps = R(1e-6), c1312 = R(13.0 / 12.0), sixth = R(1.0 / 6.0);
+  const R eps = cst<R>(1, 1e6), c1312 = cst<R>(13, 12), sixth = cst<R>(1, 6);
   R a0 = v0 - R(2) * v1 + v2, b0 = v0 - R(4) * v1 + R(3) * v2;
   R a1 = v1 - R(2) * v2 + v3, b1 = v1 - v3;
   R a2 = v2 - R(2) * v3 + v4, b2 = R(3) * v2 - R(4) * v3 + v4;
@@ -83,9 +97,9 @@ inline R weno5(R v0, R v1, R v2, R v3, R v4, R* beta_out = nullptr, R* om_out = 
   R p1 = sixth * (-v1 + R(5) * v2 + R(2) * v3);
   R p2 = sixth * (R(2) * v2 + R(5) * v3 - v4);
   R e0 = beta0 + eps, e1 = beta1 + eps, e2 = beta2 + eps;
-  R al0 = R(0.1) / (e0 * e0);
-  R al1 = R(0.6) / (e1 * e1);
-  R al2 = R(0.3) / (e2 * e2);
+  R al0 = cst<R>(1, 10) / (e0 * e0);
+  R al1 = cst<R>(6, 10) / (e1 * e1);
+  R al2 = cst<R>(3, 10) / (e2 * e2);
   R sum = al0 + al1 + al2;
   if (beta_out) { beta_out[0] = beta0; beta_out[1] = beta1; beta_out[2] = beta2; }
   if (om_out) { om_out[0] = al0 / sum; om_out[1] = al1 / sum; om_out[2] = al2 / sum; }

@@ -223,6 +223,13 @@ void compute_gradients(const Config& c, Prim<R>& P) {
   }
 }
 
+// c_p = gamma R/(gamma-1) (O1): double-rounded for double / float / the counting type (as before the
+// arbiter existed), formed in extended precision for the arbiter
+template <class R> inline R cp_of(const Config& c) { return R(c.gamma * c.Rgas / (c.gamma - 1.0)); }
+template <> inline long double cp_of<long double>(const Config& c) {
+  return (long double)c.gamma * (long double)c.Rgas / ((long double)c.gamma - 1.0L);
+}
+
 // ---------------------------------------------------------------- O6 dissipative flux of one face
 // Face on the high side of padded cell (pc[0],pc[1],pc[2]) along direction d.
 // (n,t1,t2) = (d, d+1, d+2) cyclic.  Eq. 4-5, Fourier q = -lambda grad T.
@@ -260,10 +267,10 @@ void viscous_face(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) 
   R dt2_un = i_face(g2n[0], g2n[1], g2n[2], g2n[3]);
   R dt2_ut2 = i_face(g22[0], g22[1], g22[2], g22[3]);
   R mu = viscosity(c.mu.sutherland, R(c.mu.mu_ref), R(c.mu.T_ref), R(c.mu.S), T_f);
-  R cp = R(c.gamma * c.Rgas / (c.gamma - 1.0));
+  R cp = cp_of<R>(c);
   R lambda = mu * cp / R(c.Pr);
   R div = dn_un + dt1_ut1 + dt2_ut2;
-  R tau_nn = mu * (R(2) * dn_un - R(2.0 / 3.0) * div);
+  R tau_nn = mu * (R(2) * dn_un - cst<R>(2, 3) * div);
   R tau_nt1 = mu * (dt1_un + dn_ut1);
   R tau_nt2 = mu * (dt2_un + dn_ut2);
   Fd[0] = R(0);
@@ -377,7 +384,7 @@ void rk3_step(const Config& c, R* U, R dt) {
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i)
         for (int q = 0; q < 5; ++q)
-          Un(q, i, j, k) = R(1.0 / 3.0) * Un(q, i, j, k) + R(2.0 / 3.0) * (F2(q, i, j, k) + dt * FR(q, i, j, k));
+          Un(q, i, j, k) = cst<R>(1, 3) * Un(q, i, j, k) + cst<R>(2, 3) * (F2(q, i, j, k) + dt * FR(q, i, j, k));
 }
 
 // ---------------------------------------------------------------- O9 CFL time step
@@ -413,7 +420,7 @@ int cfl_dt(const Config& c, const R* Uptr, double cfl, double* dt_out) {
       }
   if (bad) { *dt_out = std::numeric_limits<double>::quiet_NaN(); return ORA_ENOTFINITE; }
   R dt = dconv;
-  if (c.viscous) dt = s_min(dt, s_min(R(3.0 / 14.0) * dvisc, R(1.0 / 10.0) * dheat));
+  if (c.viscous) dt = s_min(dt, s_min(cst<R>(3, 14) * dvisc, cst<R>(1, 10) * dheat));
   *dt_out = cfl * (double)dt;
   return ORA_OK;
 }

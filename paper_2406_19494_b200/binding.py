@@ -36,7 +36,8 @@ class jf_disturbance(C.Structure):
 
 class jf_bc_face(C.Structure):
     _fields_ = [("type", C.c_int), ("T_wall", C.c_double), ("u_wall", C.c_double * 3),
-                ("dirichlet", c_double_p), ("dist", jf_disturbance), ("nb_width", C.c_double * 3)]
+                ("dirichlet", c_double_p), ("dist", jf_disturbance), ("nb_width", C.c_double * 3),
+                ("nb_has_face", C.c_int), ("nb_face", C.c_double * 3)]
 
 
 class jf_bc(C.Structure):
@@ -46,7 +47,7 @@ class jf_bc(C.Structure):
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
            "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
            "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
-           "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_version"]
+           "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_diag_metrics", "jf_version"]
 
 _lib = None
 
@@ -115,6 +116,8 @@ def lib():
         L.jf_diag_face_flux.restype = C.c_int
         L.jf_diag_face_flux.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(jf_mu_law),
                                         C.c_int, c_double_p, c_double_p, c_double_p, c_double_p]
+        L.jf_diag_metrics.restype = C.c_int
+        L.jf_diag_metrics.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p, c_double_p, c_double_p]
         L.jf_version.restype = C.c_char_p
         L.jf_version.argtypes = []
         _lib = L
@@ -204,6 +207,10 @@ class Solver:
             if getattr(fb, "nb_width", None) is not None:
                 for d in range(3):
                     b.nb_width[d] = float(fb.nb_width[d])
+            if getattr(fb, "nb_face", None) is not None:
+                b.nb_has_face = 1
+                for d in range(3):
+                    b.nb_face[d] = float(fb.nb_face[d])
         ga = np.asarray(case.body_accel, dtype=np.float64)
         self._keep.append(ga)
         self.stream = stream
@@ -313,6 +320,12 @@ class Solver:
         n = (C.c_ulonglong * 6)()
         self._check(lib().jf_diag_kernel_times(self.h, ms, n))
         return {lib().jf_diag_kernel_name(k).decode(): (ms[k], int(n[k])) for k in range(6)}
+
+    def jf_diag_metrics(self, axis):
+        """(1/Delta, centre, 1/(12 X_xi^c), 1/(24 X_xi^f)) of one axis as the kernels read them (padded arrays)."""
+        out = [np.zeros(self.case.n[axis] + 6) for _ in range(4)]
+        self._check(lib().jf_diag_metrics(self.h, int(axis), *[_dp(a) for a in out]))
+        return out
 
     def jf_launch_count(self):
         return int(lib().jf_launch_count(self.h))

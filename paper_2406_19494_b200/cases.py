@@ -24,6 +24,7 @@ class FaceBC:
     dirichlet: Optional[np.ndarray] = None   # prim[5][n_t2][n_t1] (rho,u,v,w,p)
     dist: Optional[dict] = None              # {"A","kappa","t1_lo","t1_hi"}  (Eq. 8)
     nb_width: Optional[tuple] = None         # BC_EXCHANGE: widths of the neighbour block's 3 nearest cells
+    nb_face: Optional[tuple] = None          # BC_EXCHANGE across an interior cut: the neighbour's 3 faces beyond this one
 
 
 @dataclass

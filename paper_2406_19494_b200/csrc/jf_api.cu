@@ -25,8 +25,9 @@ struct Metrics {
 
 // nbw[f]: for a JF_BC_EXCHANGE face f, the widths of the neighbouring block's three cells next to the
 // face (nearest first) - the halo cells then have the geometry they have on the undivided grid; else null.
+// nbf[f]: for an exchange face across an interior cut, the neighbour's three face coordinates beyond the face.
 void build_metrics(const int n[3], const double* const xf[3], const bool periodic[3], const double* const nbw[6],
-                   Metrics& M) {
+                   const double* const nbf[6], Metrics& M) {
   for (int a = 0; a < 3; ++a) {
     const int N = n[a], P = N + 2 * NH;
     std::vector<double>&d = M.dl[a], &x = M.xc[a];
@@ -40,6 +41,14 @@ void build_metrics(const int n[3], const double* const xf[3], const bool periodi
     for (int m = 1; m <= NH; ++m) { x[NH - m] = e - 0.5 * d[NH - m]; e -= d[NH - m]; }
     e = xf[a][N];
     for (int m = 1; m <= NH; ++m) { x[NH + N - 1 + m] = e + 0.5 * d[NH + N - 1 + m]; e += d[NH + N - 1 + m]; }
+    if (nbf[2 * a]) {                      // interior cut on the low side: the undivided grid's own expressions
+      double g0 = xf[a][0];
+      for (int m = 1; m <= NH; ++m) { const double g1 = nbf[2 * a][m - 1]; d[NH - m] = g0 - g1; x[NH - m] = 0.5 * (g1 + g0); g0 = g1; }
+    }
+    if (nbf[2 * a + 1]) {
+      double g0 = xf[a][N];
+      for (int m = 1; m <= NH; ++m) { const double g1 = nbf[2 * a + 1][m - 1]; d[NH + N - 1 + m] = g1 - g0; x[NH + N - 1 + m] = 0.5 * (g0 + g1); g0 = g1; }
+    }
     for (int p = NH; p < NH + N; ++p) M.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
     for (int p = NH - 1; p < NH + N; ++p) M.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
   }
@@ -98,6 +107,14 @@ struct Impl {
   double* stats;
 };
 
+}  // namespace
+namespace jf {
+inline double value_of(double a) { return a; }
+inline double value_of(float a) { return (double)a; }
+inline double value_of(Dual a) { return a.v; }
+}  // namespace jf
+namespace {
+
 bool dtype_ok(jf_dtype d) { return d == JF_F64 || d == JF_F32 || d == JF_F64_TANGENT; }
 size_t elem_size(jf_dtype d) { return d == JF_F64 ? sizeof(double) : (d == JF_F32 ? sizeof(float) : sizeof(jf::Dual)); }
 
@@ -109,6 +126,7 @@ struct jf_solver {
   Impl<float> f;
   Impl<jf::Dual> t;              // JF_F64_TANGENT: (value, tangent) pairs
   cudaStream_t stream;
+  int device;                    // the CUDA device current at jf_create: workspace, stream and every launch live there
   bool viscous;
   double Pr;
   std::string err;
@@ -147,6 +165,16 @@ struct Timed {
     cudaEventRecord(e.b, s->stream);
     s->ev_used.push_back(e);
   }
+};
+
+// Makes the solver's device current for the duration of one API call (a process driving several GPUs
+// may have another device current) and restores the caller's device on return.
+struct DeviceGuard {
+  int prev = -1; bool sw = false;
+  explicit DeviceGuard(const jf_solver* s) {
+    if (s && cudaGetDevice(&prev) == cudaSuccess && prev != s->device) sw = cudaSetDevice(s->device) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (sw) cudaSetDevice(prev); }
 };
 
 #define JF_CUDA(s, call)                                                  \
@@ -202,9 +230,14 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
   bool per[3];
   for (int a = 0; a < 3; ++a) per[a] = bc->face[2 * a].type == JF_BC_PERIODIC;
   const double* nbw[6];
-  for (int f = 0; f < 6; ++f) nbw[f] = bc->face[f].type == JF_BC_EXCHANGE ? bc->face[f].nb_width : nullptr;
+  const double* nbf[6];
+  for (int f = 0; f < 6; ++f) {
+    const bool ex = bc->face[f].type == JF_BC_EXCHANGE;
+    nbf[f] = ex && bc->face[f].nb_has_face ? bc->face[f].nb_face : nullptr;
+    nbw[f] = ex && !nbf[f] ? bc->face[f].nb_width : nullptr;
+  }
   Metrics M;
-  build_metrics(n, xf, per, nbw, M);
+  build_metrics(n, xf, per, nbw, nbf, M);
   Layout L = make_layout(n, sizeof(T));
   jf::Params<T>& P = I.P;
   for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
@@ -481,6 +514,22 @@ jf_status plane_sums(jf_solver* s, Impl<T>& I, const T* U, int axis, double* out
   return JF_OK;
 }
 
+template <class T>
+jf_status diag_metrics(jf_solver* s, Impl<T>& I, int axis, double* inv_delta, double* centre, double* i12Xc, double* i24Xf) {
+  const int Pn = I.P.P[axis];
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  std::vector<T> t(Pn);
+  const T* src[3] = {I.P.inv_dl[axis], I.P.i12Xc[axis], I.P.i24Xf[axis]};
+  double* dst[3] = {inv_delta, i12Xc, i24Xf};
+  for (int k = 0; k < 3; ++k) {
+    if (!dst[k]) continue;
+    JF_CUDA(s, cudaMemcpy(t.data(), src[k], Pn * sizeof(T), cudaMemcpyDeviceToHost));
+    for (int p = 0; p < Pn; ++p) dst[k][p] = jf::value_of(t[p]);
+  }
+  if (centre) JF_CUDA(s, cudaMemcpy(centre, I.P.xc[axis], Pn * sizeof(double), cudaMemcpyDeviceToHost));
+  return JF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -505,7 +554,13 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   for (int f = 0; f < 6; ++f) {
     const jf_bc_face& b = bc->face[f];
     if ((int)b.type < 0 || (int)b.type > 5) return JF_EINVAL;
-    if (b.type == JF_BC_EXCHANGE && !(b.nb_width[0] > 0.0 && b.nb_width[1] > 0.0 && b.nb_width[2] > 0.0)) return JF_EINVAL;
+    if (b.type == JF_BC_EXCHANGE && !b.nb_has_face && !(b.nb_width[0] > 0.0 && b.nb_width[1] > 0.0 && b.nb_width[2] > 0.0)) return JF_EINVAL;
+    if (b.type == JF_BC_EXCHANGE && b.nb_has_face) {      // strictly monotone away from the face
+      const double e = (f % 2 == 0) ? (f / 2 == 0 ? g->xf : f / 2 == 1 ? g->yf : g->zf)[0]
+                                    : (f / 2 == 0 ? g->xf[g->nx] : f / 2 == 1 ? g->yf[g->ny] : g->zf[g->nz]);
+      const double sg = (f % 2 == 0) ? -1.0 : 1.0;
+      if (!(sg * (b.nb_face[0] - e) > 0.0 && sg * (b.nb_face[1] - b.nb_face[0]) > 0.0 && sg * (b.nb_face[2] - b.nb_face[1]) > 0.0)) return JF_EINVAL;
+    }
     if (b.type == JF_BC_DIRICHLET && !b.dirichlet) return JF_EINVAL;
     if (b.type == JF_BC_WALL_ISOTHERMAL && !(b.T_wall > 0.0)) return JF_EINVAL;
   }
@@ -516,8 +571,18 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return JF_ECUDA;  // no CPU fallback
   jf_solver* s = new (std::nothrow) jf_solver();
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   s->dtype = dtype;
   s->stream = (cudaStream_t)cuda_stream;
+  if (cudaGetDevice(&s->device) != cudaSuccess) { delete s; return JF_ECUDA; }
+  {
+    // the workspace must live on the current device: the kernels are launched there
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, workspace_dev) == cudaSuccess && at.type == cudaMemoryTypeDevice && at.device != s->device) {
+      delete s;
+      return JF_EINVAL;
+    }
+  }
   s->viscous = mu->mu_ref > 0.0;
   s->Pr = Pr;
   s->launches = 0;
@@ -551,6 +616,7 @@ jf_status jf_destroy(jf_solver* s) {
 
 jf_status jf_diag_timing(jf_solver* s, int enable) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   s->timing = enable != 0;
   return JF_OK;
 }
@@ -584,6 +650,7 @@ static bool aligned16(const void* p) { return ((uintptr_t)p) % 16 == 0; }
 
 jf_status jf_fill_halo(jf_solver* s, void* U) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U) return fail(s, JF_EINVAL, "jf_fill_halo: null pointer");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_fill_halo: U not 16-byte aligned");
   return s->dtype == JF_F64   ? launch_halo<double>(s, s->d, (double*)U)
@@ -593,6 +660,7 @@ jf_status jf_fill_halo(jf_solver* s, void* U) {
 
 jf_status jf_rhs(jf_solver* s, const void* U, void* R) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !R || U == R) return fail(s, JF_EINVAL, "jf_rhs: null or aliased pointers");
   if (!aligned16(U) || !aligned16(R)) return fail(s, JF_EALIGN, "jf_rhs: pointer not 16-byte aligned");
   return s->dtype == JF_F64   ? launch_rhs<double>(s, s->d, (const double*)U, (double*)R, nullptr)
@@ -602,6 +670,7 @@ jf_status jf_rhs(jf_solver* s, const void* U, void* R) {
 
 jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_step: null pointer or NaN dt");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_step: U not 16-byte aligned");
   return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, dt)
@@ -611,6 +680,7 @@ jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
 
 jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !dt_host) return fail(s, JF_EINVAL, "jf_cfl_dt: null pointer");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_cfl_dt: U not 16-byte aligned");
   return s->dtype == JF_F64   ? cfl<double>(s, s->d, (const double*)U, cflnum, dt_host)
@@ -624,6 +694,7 @@ jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host)
 
 jf_status jf_fill_halo_axis(jf_solver* s, void* U, int axis) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_fill_halo_axis: null pointer or bad axis");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_fill_halo_axis: U not 16-byte aligned");
   return JF_DISPATCH(s, launch_halo_axis<double>(s, s->d, (double*)U, axis), launch_halo_axis<float>(s, s->f, (float*)U, axis),
@@ -638,6 +709,7 @@ size_t jf_face_elems(const jf_solver* s, int face) {
 
 jf_status jf_pack_face(jf_solver* s, const void* U, int face, void* buf) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !buf || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_pack_face: null pointer or bad face");
   return JF_DISPATCH(s, (launch_xfer<double, 0>(s, s->d, face, (double*)U, (double*)buf, nullptr, nullptr)),
                      (launch_xfer<float, 0>(s, s->f, face, (float*)U, (float*)buf, nullptr, nullptr)),
@@ -646,6 +718,7 @@ jf_status jf_pack_face(jf_solver* s, const void* U, int face, void* buf) {
 
 jf_status jf_unpack_face(jf_solver* s, void* U, int face, const void* buf) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !buf || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_unpack_face: null pointer or bad face");
   return JF_DISPATCH(s, (launch_xfer<double, 1>(s, s->d, face, (double*)U, (double*)buf, nullptr, nullptr)),
                      (launch_xfer<float, 1>(s, s->f, face, (float*)U, (float*)buf, nullptr, nullptr)),
@@ -654,6 +727,7 @@ jf_status jf_unpack_face(jf_solver* s, void* U, int face, const void* buf) {
 
 jf_status jf_pull_face(jf_solver* s, void* U, int face, const void* U_peer, const int n_peer[3]) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !U_peer || !n_peer || face < 0 || face > 5) return fail(s, JF_EINVAL, "jf_pull_face: null pointer or bad face");
   const int a = face / 2;
   const int* n = JF_DISPATCH(s, s->d.P.n, s->f.P.n, s->t.P.n);
@@ -673,6 +747,7 @@ void* jf_rk3_stage_input(jf_solver* s, void* U, int stage) {
 
 jf_status jf_rk3_stage_advance(jf_solver* s, void* U, int stage, double dt) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || stage < 1 || stage > 3 || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_stage_advance: bad argument");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_stage_advance: U not 16-byte aligned");
   return JF_DISPATCH(s, stage_advance<double>(s, s->d, (double*)U, stage, dt), stage_advance<float>(s, s->f, (float*)U, stage, dt),
@@ -681,6 +756,7 @@ jf_status jf_rk3_stage_advance(jf_solver* s, void* U, int stage, double dt) {
 
 jf_status jf_plane_sums(jf_solver* s, const void* U, int axis, double* sums) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (!U || !sums || axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_plane_sums: null pointer or bad axis");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_plane_sums: U not 16-byte aligned");
   return JF_DISPATCH(s, plane_sums<double>(s, s->d, (const double*)U, axis, sums), plane_sums<float>(s, s->f, (const float*)U, axis, sums),
@@ -689,6 +765,7 @@ jf_status jf_plane_sums(jf_solver* s, const void* U, int axis, double* sums) {
 
 jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {
   if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
   if (s->dtype != JF_F64_TANGENT) return fail(s, JF_EINVAL, "jf_set_tangent_seed: not a tangent solver");
   if (!(dA == dA) || !(dkappa == dkappa)) return fail(s, JF_EINVAL, "jf_set_tangent_seed: NaN seed");
   for (int f = 0; f < 6; ++f) { s->t.bc[f].dA = dA; s->t.bc[f].dkappa = dkappa; }
@@ -735,6 +812,15 @@ jf_status jf_diag_face_flux(jf_dtype dtype, int dir, double gamma, double R_gas,
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return JF_ECUDA;
   return dtype == JF_F64 ? diag_face_flux<double>(dir, gamma, R_gas, Pr, mu, n_faces, W, Gt, Xf, F)
                          : diag_face_flux<float>(dir, gamma, R_gas, Pr, mu, n_faces, W, Gt, Xf, F);
+}
+
+jf_status jf_diag_metrics(jf_solver* s, int axis, double* inv_delta, double* centre, double* i12Xc, double* i24Xf) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  if (axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_diag_metrics: bad axis");
+  return JF_DISPATCH(s, diag_metrics<double>(s, s->d, axis, inv_delta, centre, i12Xc, i24Xf),
+                     diag_metrics<float>(s, s->f, axis, inv_delta, centre, i12Xc, i24Xf),
+                     diag_metrics<jf::Dual>(s, s->t, axis, inv_delta, centre, i12Xc, i24Xf));
 }
 
 const char* jf_version(void) { return "libjf 0.1 (sm_100a; WENO5-JS + HLLC + 4th-order viscous + SSP-RK3)"; }

@@ -91,7 +91,14 @@ def split_case(case, blocks):
                     nb[a] = (b[a] + (-1 if side == 0 else 1)) % S[a]
                     # widths of the neighbour's three cells next to the face, nearest first (periodic wrap)
                     idx = [(lo[a] - m) % N for m in (1, 2, 3)] if side == 0 else [(hi[a] + m) % N for m in (0, 1, 2)]
-                    sub.bc.append(cases.FaceBC(cases.BC_EXCHANGE, nb_width=tuple(float(widths[a][i]) for i in idx)))
+                    # interior cut (no periodic wrap): hand over the neighbour's face coordinates, so that widths and
+                    # centres of the halo cells are the undivided grid's own expressions, bit for bit
+                    wrap = at_edge
+                    nbf = None
+                    if not wrap:
+                        nbf = tuple(float(faces[a][lo[a] - m]) for m in (1, 2, 3)) if side == 0 else \
+                            tuple(float(faces[a][hi[a] + m]) for m in (1, 2, 3))
+                    sub.bc.append(cases.FaceBC(cases.BC_EXCHANGE, nb_width=tuple(float(widths[a][i]) for i in idx), nb_face=nbf))
                     nbs.append(rank_of(nb))
                 parts.append(Part(sub, b, tuple(lo), nbs))
     return parts

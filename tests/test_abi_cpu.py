@@ -34,7 +34,7 @@ def test_struct_layouts_match_header_sizes():
     assert C.sizeof(binding.jf_grid) == 40
     assert C.sizeof(binding.jf_mu_law) == 32
     assert C.sizeof(binding.jf_disturbance) == 40
-    assert C.sizeof(binding.jf_bc_face) == 8 + 8 + 24 + 8 + 40 + 24
+    assert C.sizeof(binding.jf_bc_face) == 8 + 8 + 24 + 8 + 40 + 24 + 8 + 24   # ..., nb_width[3], nb_has_face (+pad), nb_face[3]
     assert C.sizeof(binding.jf_bc) == 6 * C.sizeof(binding.jf_bc_face)
 
 

@@ -6,13 +6,14 @@ identically ~0 carries absolute round-off eps32*|rho u|, which no fp32 code can 
 1e-3 floor); pass at 1e-10 (fp64) / 1e-4 (fp32, against the fp32 oracle).
 
 Long CFL-driven runs amplify 1-ulp differences (FMA contraction, re-associated divisions) through the
-WENO weights: the oracle moves by more than 1e-10 when ITS OWN sources are merely recompiled with
-FMA contraction (measured: 1.3e-9 in rho*v after 200 flat-plate steps).  Where that happens the test
-measures this sensitivity band with the oracle's "fma" build and requires the GPU to stay within
-BAND_FACTOR times it: the band is ONE sample of how far a legal re-rounding moves the result, the GPU
-path is another (FMA contraction plus re-associated weights and Newton reciprocals), and two such samples
-of the same amplified round-off differ by a small factor, not by orders of magnitude (DESIGN.md
-"Parity metric").  The 1e-10 bar is kept wherever the arithmetic allows it (all other variables / configs)."""
+WENO weights: on the Mach-6 plate the fp64 oracle is itself 1.1e-9 away (rho*v, 200 steps) from the
+discrete scheme's exact result.  Where GPU-vs-oracle exceeds 1e-10 for that reason the ARBITER decides:
+the oracle's own text instantiated on x87 long double (64-bit mantissa, rational constants formed in that
+precision: `ora.run_case(..., "f80")`, fed the fp64 oracle's time steps) gives the discrete result ~2000
+times more accurately than either side, and the test requires
+    |GPU - arbiter| <= max(1e-10, 2 |oracle_fp64 - arbiter|)   per conserved variable
+i.e. the GPU must be about as close to the truth as the fp64 oracle is: no free factor.  The 1e-10
+bar against the fp64 oracle itself is kept wherever the arithmetic allows it (all other variables / configs)."""
 import numpy as np
 import pytest
 
@@ -23,7 +24,6 @@ pytestmark = pytest.mark.gpu
 NH = 3
 INT = (slice(None), slice(NH, -NH), slice(NH, -NH), slice(NH, -NH))
 TOL = {"f64": 1e-10, "f32": 1e-4}
-BAND_FACTOR = 4.0
 
 
 @pytest.fixture(scope="module")
@@ -217,18 +217,27 @@ def test_cfl_dt_flags_bad_state(jf):
 
 
 # ------------------------------------------------------------------ jf_rk3_step on the configs
-def run_both(jf, ora, c, dtype="f64", n_steps=None):
+def run_both(jf, ora, c, dtype="f64", n_steps=None, want_dts=False):
     Uo, dts_o = ora.run_case(c, dtype, n_steps=n_steps)
     Ug, dts_g = jf.run_case(c, dtype, n_steps=n_steps)
     assert len(dts_o) == len(dts_g)
-    rel = max(abs(a - b) / a for a, b in zip(dts_o, dts_g)) if dts_o else 0.0
-    return metric_P(Ug.cpu().numpy(), Uo, dtype), rel, Ug, Uo
+    rel = max(abs(a - b) / a for a, b in zip(dts_o, dts_g)) if dts_o else 0.0   # |dt_gpu - dt_ora| / dt, worst step
+    err = metric_P(Ug.cpu().numpy(), Uo, dtype)
+    print(f"{c.name} {c.n} {dtype} x{len(dts_o)} steps: err {err}  max |dt_gpu-dt_ora|/dt {rel:.2e}")
+    if want_dts:
+        return err, rel, Ug, Uo, dts_o
+    return err, rel, Ug, Uo
 
 
-def sensitivity_band(ora, c, Uo, n_steps=None):
-    """How far the oracle itself moves when its sources are recompiled with FMA contraction."""
-    Uf, _ = ora.run_case(c, "f64", n_steps=n_steps, variant="fma")
-    return metric_P(Uf, Uo)
+def arbiter_check(ora, c, Ug, Uo, dts_o, label):
+    """|GPU - arbiter| <= max(1e-10, 2 |oracle_fp64 - arbiter|) per variable (module docstring).  The
+    arbiter takes the fp64 oracle's time steps, so the oracle differs from it by rounding alone."""
+    Ua, _ = ora.run_case(c, "f80", dts_in=dts_o)
+    Ua = np.asarray(Ua, dtype=np.float64)                   # rounding the arbiter to double: 1e-16, irrelevant
+    e_gpu, e_ora = metric_P(Ug, Ua), metric_P(Uo, Ua)
+    print(f"{label}: |gpu - arbiter| {e_gpu}  |oracle_fp64 - arbiter| {e_ora}")
+    assert np.all(e_gpu <= np.maximum(TOL["f64"], 2.0 * e_ora)), (e_gpu, e_ora)
+    return e_gpu, e_ora
 
 
 def test_config0_tgv32_10_steps(jf, ora):
@@ -261,26 +270,45 @@ def test_config2_channel_reduced_100_steps(jf, ora):
     assert np.all(err <= TOL["f64"]), err
 
 
-def test_config2_channel_full_size_3_steps(jf, ora):
-    err, _, _, _ = run_both(jf, ora, cases.channel(192, 128, 128), n_steps=3)
+def test_config2_channel_full_size_100_steps(jf, ora):
+    # BASELINE.json configs[2] as stated: 192 x 128 x 128, 100 RK3 steps at CFL 0.5, element by element
+    err, rel_dt, Ug, _ = run_both(jf, ora, cases.channel(192, 128, 128, n_steps=100))
+    assert rel_dt <= 1e-12
     assert np.all(err <= TOL["f64"]), err
 
 
 def test_config3_flat_plate_reduced_200_steps(jf, ora):
     c = cases.flat_plate(128, 64, 8, n_steps=200)
-    err, rel_dt, Ug, Uo = run_both(jf, ora, c)
+    err, rel_dt, Ug, Uo, dts_o = run_both(jf, ora, c, want_dts=True)
     assert rel_dt <= 1e-12
-    band = sensitivity_band(ora, c, Uo)
-    print("flat plate 200 steps: gpu-vs-oracle", err, "oracle fma-vs-nofma", band)
-    assert np.all(err <= np.maximum(TOL["f64"], BAND_FACTOR * band)), (err, band)
-    assert np.all(err[[0, 1, 4]] <= TOL["f64"]), err
+    assert np.all(err[[0, 1, 4]] <= TOL["f64"]), err         # rho, rho u, E against the fp64 oracle itself
+    arbiter_check(ora, c, Ug.cpu().numpy(), Uo, dts_o, "flat plate 128x64x8 x200")   # rho v: who is closer to the truth
     rho = Ug.cpu().numpy()[0][INT[1:]]
     assert rho.min() > 0
 
 
-def test_config3_flat_plate_full_size_5_steps(jf, ora):
-    err, _, _, _ = run_both(jf, ora, cases.flat_plate(512, 192, 8), n_steps=5)
-    assert np.all(err <= TOL["f64"]), err
+def test_config3_flat_plate_full_size_200_steps(jf, ora):
+    # BASELINE.json configs[3] as stated: 512 x 192 x 8, 200 RK3 steps at CFL 0.5, element by element.
+    # rho, rho u, E: 1e-10 against the fp64 oracle.  rho v: the arbiter (module docstring).  The case is
+    # invariant along z (8 identical periodic planes; checked bit for bit on both sides), so the arbiter
+    # runs the same case with the minimum of 4 spanwise planes and its plane is compared with every plane.
+    c = cases.flat_plate(512, 192, 8, n_steps=200)
+    err, rel_dt, Ug, Uo, dts_o = run_both(jf, ora, c, want_dts=True)
+    assert rel_dt <= 1e-12
+    assert np.all(err[[0, 1, 4]] <= TOL["f64"]), err
+    Ug = Ug.cpu().numpy()
+    assert Ug[0][INT[1:]].min() > 0
+    for U in (Ug, Uo):
+        assert all(np.array_equal(U[:, NH + k], U[:, NH]) for k in range(1, 8))
+        assert np.all(U[3][INT[1:]] == 0.0)
+    if np.all(err <= TOL["f64"]):
+        return
+    c4 = cases.flat_plate(512, 192, 4, n_steps=200)
+    Ua, _ = ora.run_case(c4, "f80", dts_in=dts_o)
+    Ua = np.repeat(np.asarray(Ua, dtype=np.float64)[:, NH:NH + 1], 8 + 2 * NH, axis=1)
+    e_gpu, e_ora = metric_P(Ug, Ua), metric_P(Uo, Ua)
+    print(f"flat plate 512x192x8 x200: |gpu - arbiter| {e_gpu}  |oracle_fp64 - arbiter| {e_ora}")
+    assert np.all(e_gpu <= np.maximum(TOL["f64"], 2.0 * e_ora)), (e_gpu, e_ora)
 
 
 def test_paper_section_3_2_boundary_layer_with_disturbance_wall(jf, ora):
@@ -294,12 +322,10 @@ def test_paper_section_3_2_boundary_layer_with_disturbance_wall(jf, ora):
     scale = np.max(np.abs(Uo), axis=(1, 2, 3), keepdims=True)
     scale[1:4] = np.max(scale[1:4])                            # rho v, rho w are ~0 here: scale by the momentum
     assert np.max(np.abs(Ug - Uo) / scale) <= 1e-13             # every halo cell
-    err, rel_dt, Ug, Uo = run_both(jf, ora, c)
+    err, rel_dt, Ug, Uo, dts_o = run_both(jf, ora, c, want_dts=True)
     assert rel_dt <= 1e-12
-    band = sensitivity_band(ora, c, Uo)
-    print("paper 3.2 case, 20 steps: gpu-vs-oracle", err, "oracle fma-vs-nofma", band)
-    assert np.all(err <= np.maximum(TOL["f64"], BAND_FACTOR * band)), (err, band)
     assert np.all(err[[0, 1, 4]] <= TOL["f64"]), err
+    arbiter_check(ora, c, Ug.cpu().numpy(), Uo, dts_o, "paper 3.2 case x20")
     # A = 0 is the plain no-slip wall on the GPU path as well, bit for bit after 3 steps
     a = cases.paper_boundary_layer(nx=60, ny=40, A=0.0)
     b = cases.paper_boundary_layer(nx=60, ny=40, disturbance=False)
@@ -313,11 +339,18 @@ def test_config4_tgv64_20_steps(jf, ora):
     assert np.all(err <= TOL["f64"]), err
 
 
-def test_config4_tgv128_2_steps_fp64_and_fp32(jf, ora):
-    err, _, _, _ = run_both(jf, ora, cases.tgv(128, n_steps=2))
+def test_config4_tgv128_20_steps_fp64_and_fp32(jf, ora):
+    # BASELINE.json configs[4] as stated: 20 RK3 steps, element by element
+    err, _, _, _ = run_both(jf, ora, cases.tgv(128, n_steps=20))
     assert np.all(err <= TOL["f64"]), err
-    err, _, _, _ = run_both(jf, ora, cases.tgv(128, n_steps=2), "f32")
+    err, _, _, _ = run_both(jf, ora, cases.tgv(128, n_steps=20), "f32")
     assert np.all(err <= TOL["f32"]), err
+
+
+def test_config4_tgv256_20_steps(jf, ora):
+    # the size bench.py times (and north_star's roofline target is quoted at), all 20 steps, element by element
+    err, _, _, _ = run_both(jf, ora, cases.tgv(256, n_steps=20))
+    assert np.all(err <= TOL["f64"]), err
 
 
 # ------------------------------------------------------------------ error behaviour of the ABI
@@ -340,42 +373,53 @@ def _sub_box_case(c, U, lo, m):
                       Pr=c.Pr, mu=c.mu, bc=cases.periodic_bc(), U0=sub, dt=c.dt, n_steps=1)
 
 
-@pytest.mark.parametrize("n,dtype", [(256, "f64"), (256, "f32"), (384, "f64"), (512, "f64"), (512, "f32")])
+@pytest.mark.parametrize("n,dtype", [(256, "f32"), (384, "f64"), (512, "f64"), (512, "f32")])
 def test_config4_full_size_sampled_against_oracle_sub_boxes(jf, ora, n, dtype):
-    """256^3 (the size bench.py times), 384^3 fp64 and 512^3 fp64 / fp32 (the largest lines of configs[4]), same
-    kernels / grids / segment lengths as bench.py launches: two RK3 steps on the GPU, then the second step
-    is checked on sampled 16^3 blocks.  One RK3 step moves information by at most 3 stages x 3 cells, so the
-    oracle stepping a periodic 40^3 cut-out of the GPU's own step-1 state is exact on the central 16^3
-    (margin 12 >= 9) whatever its (wrong) periodic wrap does at the rim.  Cut-outs are gathered on the device."""
+    """384^3 fp64 and 512^3 fp64 / fp32 (the largest lines of configs[4]; 256^3 fp64 runs all 20 steps against
+    the whole-grid oracle above), same kernels / grids / segment lengths as bench.py launches: all 20 RK3
+    steps on the GPU, and EVERY step is checked on sampled 16^3 blocks, the oracle being fed the GPU's own
+    state before that step.  One RK3 step moves information by at most 3 stages x 3 cells, so the oracle
+    stepping a periodic 40^3 cut-out of the GPU's state is exact on the central 16^3 (margin 12 >= 9)
+    whatever its (wrong) periodic wrap does at the rim.  Cut-outs are gathered on the device.  dt = 1e-3 is
+    above the linear stability limit at these sizes, so a whole-run comparison would measure
+    amplified round-off; the per-step check does not accumulate it, and the GPU state must stay finite and
+    smooth (kinetic energy within 1 % of its initial value) over the 20 steps."""
     import torch
     c = cases.tgv(n)
     s = jf.Solver(c, dtype)
     U = s.state()
-    s.jf_rk3_step(U, c.dt)
-    U1 = U.clone()
-    s.jf_rk3_step(U, c.dt)
-    torch.cuda.synchronize()
     m, g = 40, 12
     rng = np.random.default_rng(11)
     los = [(0, 0, 0), (n - 6, 3, n // 2 - 7), (100, n - 6, n - 6)] + [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(3)]
-    Ud = U.double()
-    mom = float(torch.sqrt(Ud[1] ** 2 + Ud[2] ** 2 + Ud[3] ** 2).max())
-    scale = [float(Ud[0].abs().max()), mom, mom, mom, float(Ud[4].abs().max())]
-    del Ud
+
+    def kinetic(V):
+        Vi = V[(slice(None),) + (slice(NH, -NH),) * 3].double()
+        return float(((Vi[1] ** 2 + Vi[2] ** 2 + Vi[3] ** 2) / Vi[0]).sum())
+
+    ke0 = kinetic(U)
     worst = np.zeros(5)
-    for lo in los:
-        sc = _sub_box_case(c, U1, lo, m)
-        o = ora.Oracle(sc, dtype)
-        Uo = o.state()
-        o.rk3_step(Uo, c.dt)
-        Uo = np.asarray(Uo, dtype=np.float64)
-        idx = [(np.arange(g, m - g) + lo[a]) % n + NH for a in range(3)]
-        got = _gather(U, idx)
-        ref = Uo[:, NH + g:NH + m - g, NH + g:NH + m - g, NH + g:NH + m - g]
-        for q in range(5):
-            worst[q] = max(worst[q], np.max(np.abs(got[q] - ref[q])) / scale[q])
-    print(f"tgv{n}", dtype, "sampled parity", worst)
+    for step in range(20):
+        subs = [_sub_box_case(c, U, lo, m) for lo in los]          # the GPU state before this step
+        s.jf_rk3_step(U, c.dt)
+        torch.cuda.synchronize()
+        Ud = U.double()
+        mom = float(torch.sqrt(Ud[1] ** 2 + Ud[2] ** 2 + Ud[3] ** 2).max())
+        scale = [float(Ud[0].abs().max()), mom, mom, mom, float(Ud[4].abs().max())]
+        del Ud
+        for lo, sc in zip(los, subs):
+            o = ora.Oracle(sc, dtype)
+            Uo = o.state()
+            o.rk3_step(Uo, c.dt)
+            Uo = np.asarray(Uo, dtype=np.float64)
+            idx = [(np.arange(g, m - g) + lo[a]) % n + NH for a in range(3)]
+            got = _gather(U, idx)
+            ref = Uo[:, NH + g:NH + m - g, NH + g:NH + m - g, NH + g:NH + m - g]
+            for q in range(5):
+                worst[q] = max(worst[q], np.max(np.abs(got[q] - ref[q])) / scale[q])
+    ke1 = kinetic(U)
+    print(f"tgv{n}", dtype, "sampled parity, worst of 20 steps x 6 blocks", worst, "KE ratio", ke1 / ke0)
     assert np.all(worst <= TOL[dtype]), worst
+    assert bool(torch.isfinite(U).all()) and abs(ke1 / ke0 - 1.0) < 1e-2
 
 
 # ------------------------------------------------------------------ out-of-bounds guard (compute-sanitizer is closed on this pool)

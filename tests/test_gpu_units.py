@@ -81,3 +81,44 @@ def test_face_flux_consistency_on_uniform_stencils(jf, ora):
         F = jf.jf_diag_face_flux("f64", d, G, RG, PR, mu, W)
         Fo = np.array([ora.flux_phys(d, G, W[f, 0, :5]) for f in range(n)])
         assert np.max(np.abs(F - Fo) / np.maximum(np.abs(Fo).max(axis=1, keepdims=True), 1)) <= 1e-14
+
+
+@pytest.mark.parametrize("name", ["stretched_periodic", "channel", "plate", "exchange"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_geometry_tables_against_the_oracles(jf, ora, name, dtype):
+    # reading O2: the library and the oracle each build 1/Delta, the cell centres and the index-space metrics
+    # X_xi^c, X_xi^f from the face coordinates (two independent statements of one recipe).  jf_diag_metrics
+    # copies back the tables the kernels actually read; compare them entry by entry with the oracle's.
+    from paper_2406_19494_b200 import cases, decomp
+    if name == "stretched_periodic":
+        c = cases.random_admissible(n=(13, 9, 11), seed=4, stretched=True)
+        pairs = [(c, c, [slice(None)] * 3)]
+    elif name == "channel":
+        c = cases.channel(24, 16, 16)
+        pairs = [(c, c, [slice(None)] * 3)]
+    elif name == "plate":
+        c = cases.flat_plate(64, 24, 8)
+        pairs = [(c, c, [slice(None)] * 3)]
+    else:
+        # an exchange-face block must carry the geometry of the undivided grid: compare each block's tables with
+        # the slice of the undivided oracle's tables it covers
+        c = cases.channel(24, 16, 16)
+        pairs = []
+        for part in decomp.split_case(c, (2, 2, 1)):
+            sl = [slice(part.lo[a], part.lo[a] + part.case.n[a] + 6) for a in range(3)]
+            pairs.append((part.case, c, sl))
+    tol = 4e-16 if dtype == "f64" else 2e-7
+    for blk, whole, sl in pairs:
+        s = jf.Solver(blk, dtype)
+        o = ora.Oracle(whole, "f64")
+        for a in range(3):
+            inv_dl, xc, i12Xc, i24Xf = s.jf_diag_metrics(a)
+            d, x = (v[sl[a]] for v in o.metrics(a))
+            Xc, Xf = (v[sl[a]] for v in o.metrics_index(a))
+            n = blk.n[a]
+            assert np.max(np.abs(inv_dl * d - 1.0)) <= tol
+            assert np.max(np.abs(xc - x)) <= 4e-16 * np.max(np.abs(x))      # centres are kept in fp64 for every dtype
+            ci = slice(3, n + 3)                          # X_xi^c: interior cells
+            assert np.max(np.abs(i12Xc[ci] * 12.0 * Xc[ci] - 1.0)) <= 4 * tol
+            fi = slice(2, n + 3)                          # X_xi^f: faces -1/2 .. n-1/2
+            assert np.max(np.abs(i24Xf[fi] * 24.0 * Xf[fi] - 1.0)) <= 4 * tol

@@ -241,3 +241,59 @@ def test_cfl_flags_inadmissible_state(ora):
     U = o.state()
     U[4, NH, NH, NH] = np.nan
     assert o.cfl_dt(U, 0.5)[0] == 5
+
+
+@pytest.mark.parametrize("Pr,binding", [(0.72, "heat"), (3.0, "visc")])
+def test_cfl_sutherland_two_temperature_field_closed_form(ora, Pr, binding):
+    # O9 with Sutherland viscosity: a gas at rest, uniform density, cold everywhere except a few hot cells.
+    # mu grows with T, so the hot cells set the diffusive limits: dt = cfl * 3/14 D^2 rho / mu(T_hot)
+    # (Pr = 3: the viscous limit binds) or cfl * 1/10 D^2 rho Pr / mu(T_hot) (Pr = 0.72: the heat limit),
+    # with T = p/(rho R), R != 1, and mu(T) typed here by hand from Sutherland's law.
+    n, rho, R = (6, 5, 4), 1.3, 0.4
+    T_cold, T_hot = 0.9, 2.7
+    mu_ref, T_ref, S = 0.8, 1.1, 0.35
+    c = uniform_case(n, (0.0, 0.0, 0.0), False, viscous=True, rho=rho, p=rho * R * T_cold)
+    c.R_gas, c.Pr = R, Pr
+    c.mu = {"sutherland": 1, "mu_ref": mu_ref, "T_ref": T_ref, "S": S}
+    T = np.full((n[2], n[1], n[0]), T_cold)
+    T[1, 2, 3] = T[2, 0, 5] = T_hot
+    one = np.ones_like(T)
+    c.U0 = cases.set_interior_from_prim(cases.empty_state(n), c.gamma, rho * one, 0 * one, 0 * one, 0 * one, rho * R * T)
+    d = min(c.xf[1] - c.xf[0], c.yf[1] - c.yf[0], c.zf[1] - c.zf[0])
+    mu_hot = mu_ref * (T_hot / T_ref) ** 1.5 * (T_ref + S) / (T_hot + S)
+    mu_cold = mu_ref * (T_cold / T_ref) ** 1.5 * (T_ref + S) / (T_cold + S)
+    assert mu_hot > 2 * mu_cold
+    visc, heat = 3.0 / 14.0 * d * d * rho / mu_hot, 0.1 * d * d * rho * Pr / mu_hot
+    conv = d / np.sqrt(c.gamma * R * T_hot)
+    assert (heat < visc) == (binding == "heat") and min(visc, heat) < 0.5 * conv
+    st, dt = ora.Oracle(c).cfl_dt(c.U0.copy(), 0.5)
+    assert st == 0 and dt == pytest.approx(0.5 * min(visc, heat), rel=1e-14)
+    # a constant-viscosity law on the same field gives the mu_ref limit instead
+    c.mu = {"sutherland": 0, "mu_ref": mu_ref, "T_ref": T_ref, "S": S}
+    st, dt0 = ora.Oracle(c).cfl_dt(c.U0.copy(), 0.5)
+    assert dt0 == pytest.approx(0.5 * min(3.0 / 14.0 * d * d * rho / mu_ref, 0.1 * d * d * rho * Pr / mu_ref, conv), rel=1e-14)
+
+
+# ------------------------------------------------------------------ the arbiter instantiation (x87 long double)
+def test_arbiter_is_the_same_scheme_at_higher_precision(ora):
+    # "f80" is the oracle's own text on a 64-bit mantissa.  It must (a) agree with the fp64 oracle to fp64
+    # round-off on one RHS, (b) be far closer to the truth than fp64: the fp64 oracle with and without FMA
+    # contraction are two roundings of the same scheme, so both sit at ~1e-16 of the arbiter while differing
+    # from each other by the same amount, (c) keep the exact invariants: free stream -> R == 0 bit-exactly.
+    c = cases.random_admissible(n=(10, 9, 8), seed=21, stretched=True)
+    o64, o80, ofma = ora.Oracle(c, "f64"), ora.Oracle(c, "f80"), ora.Oracle(c, "f64", variant="fma")
+    R64 = o64.rhs(o64.fill_halo(o64.state()))
+    R80 = np.asarray(o80.rhs(o80.fill_halo(o80.state())), dtype=np.float64)
+    Rf = ofma.rhs(ofma.fill_halo(ofma.state()))
+    s = np.max(np.abs(R64[INT]))
+    e64, ef, e2 = (np.max(np.abs(a[INT] - b[INT])) / s for a, b in ((R64, R80), (Rf, R80), (R64, Rf)))
+    assert 0 < e64 < 1e-13 and 0 < ef < 1e-13
+    assert e2 <= e64 + ef and e2 > 0.2 * max(e64, ef)       # the arbiter lies "between" the two roundings
+    u = uniform_case((7, 6, 5), (0.7, -0.4, 0.25), True)
+    o = ora.Oracle(u, "f80")
+    assert np.max(np.abs(o.rhs(o.fill_halo(o.state()))[INT])) == 0.0
+    # one quantity known in closed form to all digits: 1/3, 2/3 of the last RK3 stage are formed in long double
+    # (a double-rounded 1/3 would leave an error of 1.85e-17 U): U' = 1/3 U + 2/3 (U + dt*0) must return U to 1 ulp80
+    U1 = o.rk3_step(o.state(), 1e-2)
+    U0 = np.asarray(u.U0, dtype=np.longdouble)
+    assert np.max(np.abs(U1[INT] - U0[INT]) / np.abs(U0[INT]).max()) <= 2.0 ** -62
