@@ -136,6 +136,25 @@ jf_status jf_rk3_step(jf_solver *s, void *U_dev, double dt);
  * interior cell is non-finite or has rho <= 0 or p <= 0. */
 jf_status jf_cfl_dt(jf_solver *s, const void *U_dev, double cfl, double *dt_host);
 
+/* Device-resident time step: the same reduction, finished on the device (the last block forms dt), with NO host
+ * synchronisation:   dt = min(jf_cfl_dt's value, t_end - t)   (t_end = NaN: no clipping),
+ * stored in the solver's workspace together with the running time t <- t + dt (t starts at 0; jf_dev_time sets it).
+ * jf_rk3_step_dev then advances U by that dt (its z + RK kernels read it from device memory), so a CFL-driven loop
+ *     for (...) { jf_cfl_dt_dev(s, U, cfl, t_end); jf_rk3_step_dev(s, U); }
+ * queues steps without ever waiting for the GPU; the host reads dt and t when it wants them (jf_dev_time), e.g.
+ * one step late.  An inadmissible state makes dt NaN (it then spreads through U) and jf_dev_time returns
+ * JF_ENOTFINITE from then on.  Asynchronous. */
+jf_status jf_cfl_dt_dev(jf_solver *s, const void *U_dev, double cfl, double t_end);
+jf_status jf_rk3_step_dev(jf_solver *s, void *U_dev);
+/* set == 0: synchronise, then *dt_host = last device-side dt, *t_host = device-side time (either may be NULL).
+ * set != 0: device-side time <- *t_host, dt <- 0, status cleared. */
+jf_status jf_dev_time(jf_solver *s, int set, double *dt_host, double *t_host);
+
+/* Launch mechanics of jf_rk3_step / jf_rk3_step_dev: the 15 launches of a step are captured once per state-array
+ * address into a CUDA graph owned by the solver (on a private stream) and replayed into the caller's stream; their
+ * z + RK kernels read dt from the device scalar, which jf_rk3_step sets with a one-thread kernel.  Environment
+ * JF_GRAPH=0 at jf_create time turns this off (plain launches; also used while jf_diag_timing is on). */
+
 /* ---- Block decomposition ------------------------------------------
  * One solver per block; faces between blocks are JF_BC_EXCHANGE.  One RK stage of a decomposed step is
  *   for axis in x, y, z:   every block: jf_fill_halo_axis(axis)            (its physical faces)

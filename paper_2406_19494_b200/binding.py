@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libjf.so")
+# JF_LIB: load another build of the same library (e.g. one compiled with different tuning macros)
+LIB_PATH = os.environ.get("JF_LIB") or os.path.join(_HERE, "libjf.so")
 
 JF_OK, JF_EINVAL, JF_EALIGN, JF_EWORKSPACE, JF_ECUDA, JF_ENOTFINITE = range(6)
 JF_F64, JF_F32, JF_F64_TANGENT = 0, 1, 2
@@ -45,7 +46,7 @@ class jf_bc(C.Structure):
 
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
-           "jf_rk3_step", "jf_cfl_dt", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
+           "jf_rk3_step", "jf_cfl_dt", "jf_cfl_dt_dev", "jf_rk3_step_dev", "jf_dev_time", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
            "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_diag_metrics", "jf_version"]
 
@@ -101,6 +102,12 @@ def lib():
         L.jf_rk3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
         L.jf_cfl_dt.restype = C.c_int
         L.jf_cfl_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_double, c_double_p]
+        L.jf_cfl_dt_dev.restype = C.c_int
+        L.jf_cfl_dt_dev.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double]
+        L.jf_rk3_step_dev.restype = C.c_int
+        L.jf_rk3_step_dev.argtypes = [C.c_void_p, C.c_void_p]
+        L.jf_dev_time.restype = C.c_int
+        L.jf_dev_time.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p]
         L.jf_last_error.restype = C.c_char_p
         L.jf_last_error.argtypes = [C.c_void_p]
         L.jf_launch_count.restype = C.c_ulonglong
@@ -311,6 +318,22 @@ class Solver:
         st = lib().jf_cfl_dt(self.h, self._ptr(U), float(cfl), C.byref(dt))
         return st, dt.value
 
+    def jf_cfl_dt_dev(self, U, cfl, t_end=None):
+        self._check(lib().jf_cfl_dt_dev(self.h, self._ptr(U), float(cfl), float("nan") if t_end is None else float(t_end)))
+
+    def jf_rk3_step_dev(self, U):
+        self._check(lib().jf_rk3_step_dev(self.h, self._ptr(U)))
+        return U
+
+    def jf_dev_time(self, set_t=None):
+        """(status, dt, t) of the device-side clock (synchronises); set_t: reset the clock to that time first."""
+        dt, t = C.c_double(), C.c_double()
+        if set_t is not None:
+            t.value = float(set_t)
+            self._check(lib().jf_dev_time(self.h, 1, None, C.byref(t)))
+        st = lib().jf_dev_time(self.h, 0, C.byref(dt), C.byref(t))
+        return st, dt.value, t.value
+
     def jf_diag_timing(self, enable):
         self._check(lib().jf_diag_timing(self.h, int(bool(enable))))
 
@@ -331,13 +354,30 @@ class Solver:
         return int(lib().jf_launch_count(self.h))
 
 
-def run_case(case, dtype="f64", n_steps=None, device="cuda:0", solver=None):
+def run_case(case, dtype="f64", n_steps=None, device="cuda:0", solver=None, device_dt=False):
     """Advance a case on the GPU the way the drivers do (mirror of the oracle-side driver in
-    tests): fixed dt x n_steps, or CFL steps clipped to t_end.  Returns (U tensor, list of dt)."""
+    tests): fixed dt x n_steps, or CFL steps clipped to t_end.  Returns (U tensor, list of dt).
+    device_dt: CFL-driven cases take jf_cfl_dt_dev + jf_rk3_step_dev (the step never leaves the device);
+    dt is read back after each step only to report it and to detect t_end."""
     s = solver or Solver(case, dtype, device)
     U = s.state()
     dts, t, step = [], 0.0, 0
     n = n_steps if n_steps is not None else case.n_steps
+    if device_dt and case.dt is None:
+        s.jf_dev_time(set_t=0.0)
+        while True:
+            if n is not None and step >= n:
+                break
+            if case.t_end is not None and t >= case.t_end * (1 - 1e-14):
+                break
+            s.jf_cfl_dt_dev(U, case.cfl, case.t_end)
+            s.jf_rk3_step_dev(U)
+            st, dt, t = s.jf_dev_time()
+            if st != JF_OK:
+                raise JFError(st, f"jf_cfl_dt_dev at step {step}")
+            dts.append(dt)
+            step += 1
+        return U, dts
     while True:
         if n is not None and step >= n:
             break

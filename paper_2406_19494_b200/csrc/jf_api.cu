@@ -10,6 +10,9 @@
 #include <cuda_runtime.h>
 #include "../../include/jf.h"
 #include "jf_kernels.cuh"
+#include "jf_tma.cuh"
+#include <cstdlib>
+#include <unordered_map>
 
 namespace {
 
@@ -58,7 +61,7 @@ struct Layout {  // byte offsets into the workspace
   size_t tab_T[3][4];   // inv_dl, dl, i12Xc, i24Xf per axis (dtype)
   size_t tab_xc[3];     // double
   size_t dirichlet[6];  // double
-  size_t cfl;           // 4 x u64
+  size_t cfl;           // 8 x u64: three minima, flag, block counter, then (as doubles) dt, t, and a sticky status word
   size_t stats;         // NSTAT x max(n) x STATS_NB doubles (plane-sum partials)
   size_t R, A, B, G;    // fields (dtype)
   size_t total;
@@ -75,7 +78,7 @@ Layout make_layout(const int n[3], size_t esz) {
     int a = f / 2, t1 = (a == 0) ? 1 : 0, t2 = (a == 2) ? 1 : 2;
     L.dirichlet[f] = off; off = align_up(off + (size_t)5 * n[t1] * n[t2] * sizeof(double));
   }
-  L.cfl = off; off = align_up(off + 4 * sizeof(unsigned long long));
+  L.cfl = off; off = align_up(off + 8 * sizeof(unsigned long long));
   L.stats = off; off = align_up(off + (size_t)jf::NSTAT * std::max(n[0], std::max(n[1], n[2])) * STATS_NB * sizeof(double));
   size_t vol = (size_t)(n[0] + 6) * (n[1] + 6) * (n[2] + 6);
   L.R = off; off = align_up(off + 5 * vol * esz);
@@ -132,6 +135,16 @@ struct jf_solver {
   std::string err;
   unsigned long long launches;
   int seg_len[3];
+  // TMA-staged gradient pass (jf_tma.cuh): tensor maps per state-array base address (U, stage buffers A, B, ...)
+  bool grad_tma = false;
+  std::unordered_map<const void*, CUtensorMap> maps;
+  // CUDA graphs of one RK3 step (the 15 launches), one per state-array address, captured on first use on a private
+  // stream and launched into the caller's stream.  The kernels of a graph read dt from the device scalar
+  // (RKArgs::dt_dev), so the same graph serves every dt (jf_rk3_step sets it, jf_cfl_dt_dev computes it).
+  bool use_graph = true;
+  cudaStream_t cap_stream = nullptr;
+  struct GraphEntry { const void* U; cudaGraphExec_t exec; unsigned kernels; };
+  std::vector<GraphEntry> graphs;
   // optional per-kernel timing (jf_diag_timing): CUDA events around every launch
   bool timing = false;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -277,6 +290,11 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
   }
   I.R = (T*)(ws + L.R); I.A = (T*)(ws + L.A); I.B = (T*)(ws + L.B); I.G = (T*)(ws + L.G);
   I.cfl_out = (unsigned long long*)(ws + L.cfl);
+  {
+    // armed once; every finalising reduction re-arms it (jf_cfl_dt_dev), jf_cfl_dt re-arms by memset
+    unsigned long long h[8] = {~0ULL, ~0ULL, ~0ULL, 0, 0, 0, 0, 0};
+    JF_CUDA(s, cudaMemcpy(I.cfl_out, h, sizeof(h), cudaMemcpyHostToDevice));
+  }
   I.stats = (double*)(ws + L.stats);
   return JF_OK;
 }
@@ -386,6 +404,58 @@ jf_status launch_xfer(jf_solver* s, Impl<T>& I, int face, T* U, T* buf, const T*
   return JF_OK;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return (EncodeTiledFn)f;
+  }();
+  return fn;
+}
+
+// Tensor map of one state array U[5][Pz][Py][Px] (x fastest) for boxes {GM_SX, GM_SY, 1, 4}: the (x,y) tile of one
+// plane with its 2-cell rim, variables rho .. rho w.  Out-of-range box cells are zero-filled.  Cached per base address.
+template <class T>
+const CUtensorMap* grad_map(jf_solver* s, const jf::Params<T>& P, const T* U) {
+  auto it = s->maps.find((const void*)U);
+  if (it != s->maps.end()) return &it->second;
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return nullptr;
+  CUtensorMap m;
+  const cuuint64_t dims[4] = {(cuuint64_t)P.P[0], (cuuint64_t)P.P[1], (cuuint64_t)P.P[2], 5};
+  const cuuint64_t strides[3] = {(cuuint64_t)P.sy * sizeof(T), (cuuint64_t)P.sz * sizeof(T), (cuuint64_t)P.vol * sizeof(T)};
+  const cuuint32_t box[4] = {(cuuint32_t)jf::GM_SX, (cuuint32_t)jf::GM_SY, 1, 4};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUtensorMapDataType dt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  if (enc(&m, dt, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return nullptr;
+  if (s->maps.size() > 64) s->maps.clear();
+  return &(s->maps[(const void*)U] = m);
+}
+template <>
+const CUtensorMap* grad_map<jf::Dual>(jf_solver*, const jf::Params<jf::Dual>&, const jf::Dual*) { return nullptr; }
+template <>
+const CUtensorMap* grad_map<float>(jf_solver*, const jf::Params<float>&, const float*) { return nullptr; }
+
+template <class T>
+bool launch_grad_tma(jf_solver* s, Impl<T>& I, const T* U, dim3 grid, int Lz) {
+  const CUtensorMap* m = grad_map<T>(s, I.P, U);
+  if (!m) return false;
+  jf::gradient_tma_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), sizeof(jf::GradTmaSmem<T>), s->stream>>>(I.P, *m, I.G, Lz);
+  return true;
+}
+template <>
+bool launch_grad_tma<jf::Dual>(jf_solver*, Impl<jf::Dual>&, const jf::Dual*, dim3, int) { return false; }
+template <>
+bool launch_grad_tma<float>(jf_solver*, Impl<float>&, const float*, dim3, int) { return false; }
+
 // R_NSE of Eq. 6.  rk == nullptr: R <- R_NSE(U).  Otherwise the z sweep applies the RK stage.
 template <class T, bool VISC>
 jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
@@ -400,7 +470,8 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
     if (nseg < 1) nseg = 1;
     const int Lz = (P.P[2] + nseg - 1) / nseg;
     dim3 grid((P.P[0] + jf::GM_TX - 1) / jf::GM_TX, (P.P[1] + jf::GM_TY - 1) / jf::GM_TY, (P.P[2] + Lz - 1) / Lz);
-    jf::gradient_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
+    if (!(s->grad_tma && launch_grad_tma<T>(s, I, U, grid, Lz)))
+      jf::gradient_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
     s->launches += 1;
   }
   {
@@ -409,9 +480,9 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
     const size_t sh = (size_t)jf::XS_WARPS * (jf::XS<VISC>::NV * jf::XS_RING + jf::XS_CARRY) * sizeof(T);
     jf::sweep_x_kernel<T, VISC><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
-  const size_t sh = (size_t)jf::YZ_RING * jf::YZ<VISC>::NP * jf::YZ_TX * jf::YZ_TY * sizeof(jf::Pair2<T>);
+  const size_t sh = jf::yz_smem_bytes<T, VISC>();
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
-  jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0)};
+  jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0), nullptr};
   {
     Timed t(s, K_SWEEP_Y);
     const int L = s->seg_len[1];
@@ -434,10 +505,15 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
 // 128-thread block in fp64): above the 48 KB default, so opt in once per solver.
 template <class T, bool VISC>
 cudaError_t opt_in_smem() {
-  const int sh = (int)((size_t)jf::YZ_RING * jf::YZ<VISC>::NP * jf::YZ_TX * jf::YZ_TY * sizeof(jf::Pair2<T>));
+  const int sh = (int)jf::yz_smem_bytes<T, VISC>();
   cudaError_t e = cudaSuccess;
   auto set = [&](const void* f) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
+#ifdef JF_YZ_CARVEOUT
+    // (measured: with the largest carve-out the L1 shrinks and the re-read of U_s in the z + RK sweep misses it:
+    // z + RK 2.15 -> 2.93 ms per step at 256^3; the default carve-out is kept)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, JF_YZ_CARVEOUT);
+#endif
   };
   set((const void*)jf::sweep_yz_kernel<T, 1, VISC, 0>);
   set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 1>);
@@ -457,37 +533,99 @@ template <class T>
 T* stage_input(Impl<T>& I, T* U, int stage) { return stage == 1 ? U : (stage == 2 ? I.A : I.B); }
 
 template <class T>
-jf_status stage_advance(jf_solver* s, Impl<T>& I, T* U, int stage, double dt) {
-  if (stage == 1) { jf::RKArgs<T> r{U, I.A, T(0), T(1), T(dt)}; return launch_rhs<T>(s, I, U, I.R, &r); }
-  if (stage == 2) { jf::RKArgs<T> r{U, I.B, T(0.75), T(0.25), T(dt)}; return launch_rhs<T>(s, I, I.A, I.R, &r); }
-  jf::RKArgs<T> r{U, U, T(1.0 / 3.0), T(2.0 / 3.0), T(dt)};
+jf_status stage_advance(jf_solver* s, Impl<T>& I, T* U, int stage, double dt, const double* dt_dev = nullptr) {
+  if (stage == 1) { jf::RKArgs<T> r{U, I.A, T(0), T(1), T(dt), dt_dev}; return launch_rhs<T>(s, I, U, I.R, &r); }
+  if (stage == 2) { jf::RKArgs<T> r{U, I.B, T(0.75), T(0.25), T(dt), dt_dev}; return launch_rhs<T>(s, I, I.A, I.R, &r); }
+  jf::RKArgs<T> r{U, U, T(1.0 / 3.0), T(2.0 / 3.0), T(dt), dt_dev};
   return launch_rhs<T>(s, I, I.B, I.R, &r);
 }
 
 template <class T>
-jf_status rk3(jf_solver* s, Impl<T>& I, T* U, double dt) {
+jf_status rk3_launches(jf_solver* s, Impl<T>& I, T* U, double dt, const double* dt_dev) {
   jf_status st;
   for (int stage = 1; stage <= 3; ++stage) {
     if ((st = launch_halo<T>(s, I, stage_input<T>(I, U, stage)))) return st;
-    if ((st = stage_advance<T>(s, I, U, stage, dt))) return st;
+    if ((st = stage_advance<T>(s, I, U, stage, dt, dt_dev))) return st;
   }
+  return JF_OK;
+}
+
+__global__ void set_dt_kernel(double* st, double dt) { st[5] = dt; }
+
+// One RK3 step.  dev_dt: take the step from the device scalar cfl_out[5] (jf_cfl_dt_dev) instead of `dt`.
+// With graphs on (default; off while per-launch timing is enabled) the 15 launches are replayed from a graph whose
+// kernels read the device scalar; a host dt is written there first by a one-thread kernel.
+template <class T>
+jf_status rk3(jf_solver* s, Impl<T>& I, T* U, double dt, bool dev_dt) {
+  double* dt_dev = reinterpret_cast<double*>(I.cfl_out) + 5;
+  if (!s->use_graph || s->timing) return rk3_launches<T>(s, I, U, dt, dev_dt ? dt_dev : nullptr);
+  jf_solver::GraphEntry* ge = nullptr;
+  for (auto& g : s->graphs)
+    if (g.U == (const void*)U) ge = &g;
+  if (!ge) {
+    if (!s->cap_stream) JF_CUDA(s, cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+    const cudaStream_t user = s->stream;
+    const unsigned long long l0 = s->launches;
+    JF_CUDA(s, cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    s->stream = s->cap_stream;
+    const jf_status st = rk3_launches<T>(s, I, U, 0.0, dt_dev);
+    s->stream = user;
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(s->cap_stream, &graph);
+    const unsigned nk = (unsigned)(s->launches - l0);
+    s->launches = l0;
+    if (st != JF_OK) { if (graph) cudaGraphDestroy(graph); return st; }
+    if (ce != cudaSuccess) return fail(s, JF_ECUDA, "cudaStreamEndCapture", ce);
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ci = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ci != cudaSuccess) return fail(s, JF_ECUDA, "cudaGraphInstantiate", ci);
+    if (s->graphs.size() >= 8) { cudaGraphExecDestroy(s->graphs.front().exec); s->graphs.erase(s->graphs.begin()); }
+    s->graphs.push_back({(const void*)U, exec, nk});
+    ge = &s->graphs.back();
+  }
+  if (!dev_dt) {
+    set_dt_kernel<<<1, 1, 0, s->stream>>>(reinterpret_cast<double*>(I.cfl_out), dt);
+    s->launches += 1;
+  }
+  JF_CUDA(s, cudaGraphLaunch(ge->exec, s->stream));
+  s->launches += ge->kernels;
+  return JF_OK;
+}
+
+template <class T>
+int cfl_blocks(const Impl<T>& I) {
+  const long long ncell = (long long)I.P.n[0] * I.P.n[1] * I.P.n[2];
+  return (int)std::min<long long>((ncell + 255) / 256, 148LL * 8);
+}
+
+// reduction + finalize on the device (no host synchronisation): dt -> cfl_out[5], t += dt -> cfl_out[6]
+template <class T>
+jf_status cfl_dev(jf_solver* s, Impl<T>& I, const T* U, double cflnum, double t_end) {
+  {
+    Timed t(s, K_CFL);
+    jf::cfl_kernel<T><<<cfl_blocks<T>(I), 256, 0, s->stream>>>(I.P, U, I.cfl_out, 1, cflnum, t_end);
+  }
+  s->launches += 1;
+  JF_CUDA(s, cudaPeekAtLastError());
   return JF_OK;
 }
 
 template <class T>
 jf_status cfl(jf_solver* s, Impl<T>& I, const T* U, double cflnum, double* dt_host) {
   JF_CUDA(s, cudaMemsetAsync(I.cfl_out, 0xFF, 3 * sizeof(unsigned long long), s->stream));
-  JF_CUDA(s, cudaMemsetAsync(I.cfl_out + 3, 0, sizeof(unsigned long long), s->stream));
-  long long ncell = (long long)I.P.n[0] * I.P.n[1] * I.P.n[2];
-  int blocks = (int)std::min<long long>((ncell + 255) / 256, 148LL * 8);
+  JF_CUDA(s, cudaMemsetAsync(I.cfl_out + 3, 0, 2 * sizeof(unsigned long long), s->stream));
+  int blocks = cfl_blocks<T>(I);
   {
     Timed t(s, K_CFL);
-    jf::cfl_kernel<T><<<blocks, 256, 0, s->stream>>>(I.P, U, I.cfl_out);
+    jf::cfl_kernel<T><<<blocks, 256, 0, s->stream>>>(I.P, U, I.cfl_out, 0, 0.0, 0.0);
   }
   s->launches += 1;
   JF_CUDA(s, cudaPeekAtLastError());
   unsigned long long h[4];
   JF_CUDA(s, cudaMemcpyAsync(h, I.cfl_out, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  JF_CUDA(s, cudaMemsetAsync(I.cfl_out, 0xFF, 3 * sizeof(unsigned long long), s->stream));   // leave it armed for jf_cfl_dt_dev
+  JF_CUDA(s, cudaMemsetAsync(I.cfl_out + 3, 0, 2 * sizeof(unsigned long long), s->stream));
   JF_CUDA(s, cudaStreamSynchronize(s->stream));
   if (h[3]) { *dt_host = std::nan(""); return fail(s, JF_ENOTFINITE, "jf_cfl_dt: non-finite state or rho <= 0 or p <= 0"); }
   double v[3];
@@ -596,6 +734,27 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
                                        : (s->viscous ? opt_in_smem<jf::Dual, true>() : opt_in_smem<jf::Dual, false>());
     if (ce != cudaSuccess) { delete s; return JF_ECUDA; }
   }
+  {
+    // TMA needs 16-byte global strides: (nx+6) * 8 bytes, i.e. even nx.  fp64 only: the tangent type has no tensor-map
+    // data type, and the fp32 instantiation (pitch aligned only for nx = 2 mod 4) faulted on the box copy in the one
+    // run it got ("illegal instruction", 70x35x67) and is not worth a second kernel.
+    // JF_GRAD_TMA=0/1 overrides the default (tuning / A-B measurements).
+    const size_t esz = elem_size(dtype);
+    bool ok = dtype == JF_F64 && ((size_t)(g->nx + 6) * esz) % 16 == 0 && encode_tiled_fn() != nullptr;
+    const char* e = std::getenv("JF_GRAD_TMA");
+#ifdef JF_GRAD_TMA_DEFAULT
+    bool want = JF_GRAD_TMA_DEFAULT != 0;
+#else
+    bool want = false;
+#endif
+    if (e) want = std::atoi(e) != 0;
+    s->grad_tma = ok && want;
+    if (s->grad_tma) {
+      cudaError_t ce = cudaFuncSetAttribute((const void*)jf::gradient_tma_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(jf::GradTmaSmem<double>));
+      if (ce != cudaSuccess) s->grad_tma = false;
+    }
+  }
+  if (const char* e = std::getenv("JF_GRAPH")) s->use_graph = std::atoi(e) != 0;
   const int n[3] = {g->nx, g->ny, g->nz};
   s->seg_len[0] = 0;
   auto cdiv = [](int a, int b) { return (long long)((a + b - 1) / b); };
@@ -609,6 +768,8 @@ jf_status jf_destroy(jf_solver* s) {
   if (s) {
     for (auto& e : s->ev_used) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (auto& e : s->ev_free) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (auto& g : s->graphs) cudaGraphExecDestroy(g.exec);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
   }
   delete s;
   return JF_OK;
@@ -673,9 +834,50 @@ jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
   DeviceGuard dev_guard(s);
   if (!U || !(dt == dt)) return fail(s, JF_EINVAL, "jf_rk3_step: null pointer or NaN dt");
   if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_step: U not 16-byte aligned");
-  return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, dt)
-         : s->dtype == JF_F32 ? rk3<float>(s, s->f, (float*)U, dt)
-                              : rk3<jf::Dual>(s, s->t, (jf::Dual*)U, dt);
+  return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, dt, false)
+         : s->dtype == JF_F32 ? rk3<float>(s, s->f, (float*)U, dt, false)
+                              : rk3<jf::Dual>(s, s->t, (jf::Dual*)U, dt, false);
+}
+
+jf_status jf_cfl_dt_dev(jf_solver* s, const void* U, double cflnum, double t_end) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  if (!U || !(cflnum > 0.0)) return fail(s, JF_EINVAL, "jf_cfl_dt_dev: null pointer or cfl <= 0");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_cfl_dt_dev: U not 16-byte aligned");
+  return s->dtype == JF_F64   ? cfl_dev<double>(s, s->d, (const double*)U, cflnum, t_end)
+         : s->dtype == JF_F32 ? cfl_dev<float>(s, s->f, (const float*)U, cflnum, t_end)
+                              : cfl_dev<jf::Dual>(s, s->t, (const jf::Dual*)U, cflnum, t_end);
+}
+
+jf_status jf_rk3_step_dev(jf_solver* s, void* U) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  if (!U) return fail(s, JF_EINVAL, "jf_rk3_step_dev: null pointer");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_rk3_step_dev: U not 16-byte aligned");
+  return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, 0.0, true)
+         : s->dtype == JF_F32 ? rk3<float>(s, s->f, (float*)U, 0.0, true)
+                              : rk3<jf::Dual>(s, s->t, (jf::Dual*)U, 0.0, true);
+}
+
+jf_status jf_dev_time(jf_solver* s, int set, double* dt_host, double* t_host) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  unsigned long long* out = s->dtype == JF_F64 ? s->d.cfl_out : s->dtype == JF_F32 ? s->f.cfl_out : s->t.cfl_out;
+  if (set) {
+    if (!t_host) return fail(s, JF_EINVAL, "jf_dev_time: null pointer");
+    unsigned long long h[3] = {0, 0, 0};
+    std::memcpy(&h[1], t_host, sizeof(double));
+    JF_CUDA(s, cudaMemcpyAsync(out + 5, h, sizeof(h), cudaMemcpyHostToDevice, s->stream));
+    JF_CUDA(s, cudaStreamSynchronize(s->stream));
+    return JF_OK;
+  }
+  unsigned long long h[3];
+  JF_CUDA(s, cudaMemcpyAsync(h, out + 5, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  if (dt_host) std::memcpy(dt_host, &h[0], sizeof(double));
+  if (t_host) std::memcpy(t_host, &h[1], sizeof(double));
+  if (h[2]) return fail(s, JF_ENOTFINITE, "jf_dev_time: a device-side CFL reduction met a non-finite state or rho <= 0 or p <= 0");
+  return JF_OK;
 }
 
 jf_status jf_cfl_dt(jf_solver* s, const void* U, double cflnum, double* dt_host) {

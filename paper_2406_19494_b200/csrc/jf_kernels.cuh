@@ -395,6 +395,8 @@ struct RKArgs {
   const T* Un;   // U^n
   T* Uout;       // stage output
   T a, b, dt;    // U_out = a U^n + b (U_s + dt R)
+  const double* dt_dev;   // if not null: the time step is read from device memory (written by cfl_kernel's finalize:
+                          // jf_cfl_dt_dev), not taken from `dt`: no host round trip between the CFL reduction and the step
 };
 
 // ------------------------------------------------------------------ x sweep
@@ -462,10 +464,10 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
   T raw[5], gn[3] = {T(0), T(0), T(0)};
   auto fetch = [&](bool in) {                // the cell at (base, p); `in`: inside this warp's stream
 #pragma unroll
-    for (int q = 0; q < 5; ++q) raw[q] = in ? (U + q * P.vol)[base + (unsigned)p] : T(1);
+    for (int q = 0; q < 5; ++q) raw[q] = in ? ld_stream((U + q * P.vol) + (base + (unsigned)p)) : T(1);
     if (VISC) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) gn[c] = in ? gsrc[c][base + (unsigned)p] : T(0);
+      for (int c = 0; c < 3; ++c) gn[c] = in ? ld_stream(gsrc[c] + (base + (unsigned)p)) : T(0);
     }
   };
   fetch(lane < S);
@@ -538,7 +540,7 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     if (upd) {
       const unsigned oc = cbase + (unsigned)(pc - 1);
 #pragma unroll
-      for (int q = 0; q < 5; ++q) (R + q * P.vol)[oc] = dF[q];
+      for (int q = 0; q < 5; ++q) st_stream((R + q * P.vol) + oc, dF[q]);
     }
     __syncwarp();
   }
@@ -564,6 +566,14 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 #endif
 constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY, YZ_RING = 5;
 template <bool VISC> struct YZ { static constexpr int NP = VISC ? 5 : 3; };   // pairs per window cell
+template <class T, bool VISC>
+constexpr size_t yz_smem_bytes() {
+  size_t b = (size_t)YZ_RING * YZ<VISC>::NP * YZ_TX * YZ_TY * sizeof(Pair2<T>);
+#ifdef JF_YZ_FSMEM
+  b += (size_t)5 * YZ_TX * YZ_TY * sizeof(T);
+#endif
+  return b;
+}
 template <class T, int DIR, bool VISC, int MODE>
 __global__ void __launch_bounds__(YZ_TX * YZ_TY, sizeof(T) == 4 ? JF_YZ_MINB_F32 : JF_YZ_MINB)
 sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* R, RKArgs<T> rk, int L) {
@@ -596,7 +606,8 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       P2* dst = mine + slot * (NP * NT);
       dst[0] = P2{W[0], W[1]};
       dst[NT] = P2{W[2], W[3]};
-      dst[2 * NT] = P2{W[4], W[5]};
+      if (VISC) dst[2 * NT] = P2{W[4], W[5]};
+      else dst[2 * NT].a = W[4];             // inviscid: the T word is not used (JF_YZ_XCHG keeps W^- there)
       if (VISC) {
         dst[3 * NT] = P2{gn[0], gn[1]};
         dst[4 * NT].a = gn[2];
@@ -621,16 +632,38 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     for (int s = 0; s < YZ_RING; ++s) {
       const unsigned o = col + (unsigned)(c0 + s) * sm;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raws[s][q] = (U + q * P.vol)[o];
+      for (int q = 0; q < 5; ++q) raws[s][q] = (MODE == 2) ? (U + q * P.vol)[o] : ld_stream((U + q * P.vol) + o);
 #pragma unroll
-      for (int c = 0; c < 3; ++c) gns[s][c] = VISC ? gsrc[c][o] : T(0);
+      for (int c = 0; c < 3; ++c) gns[s][c] = VISC ? ld_stream(gsrc[c] + o) : T(0);
     }
 #pragma unroll
     for (int s = 0; s < YZ_RING; ++s) put(s, raws[s], gns[s]);
   }
-  T WmPrev[5], Fprev[5];
+  // W^-_{c+1/2} of the previous step and (JF_YZ_FSMEM) the previous face flux are handed from step to step through
+  // thread-private shared memory instead of registers: variable q lives in the unused tenth value of ring slot q
+  // (the flux in five more words after the ring).  20 (40) registers and the 10 (20) rotation moves per step go.
+#ifdef JF_YZ_XCHG
+  auto xw = [&](int q) -> T* {
+    if (PAIR) return &(mine + q * (NP * NT) + (NP - 1) * NT)->b;
+    return mine1 + q * (2 * NP * NT) + (2 * NP - 1) * NT;
+  };
+  static_assert(!VISC || NP == 5, "pad slot");
 #pragma unroll
-  for (int q = 0; q < 5; ++q) { WmPrev[q] = T(1); Fprev[q] = T(0); }
+  for (int q = 0; q < 5; ++q) *xw(q) = T(1);
+#else
+  T WmPrev[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) WmPrev[q] = T(1);
+#endif
+#ifdef JF_YZ_FSMEM
+  T* fsm = reinterpret_cast<T*>(smem_raw + (size_t)YZ_RING * NP * NT * sizeof(P2)) + tid;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) fsm[q * NT] = T(0);
+#else
+  T Fprev[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Fprev[q] = T(0);
+#endif
   int s0 = 0;                                // slot of cell c-2
   // metric table entries of the face / cell the NEXT step treats, loaded one step ahead (a per-step
   // scalar load issued where it is used stalls the warp for an L2 round trip: 11-13 % of all stall samples)
@@ -658,6 +691,11 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     };
     T Wm[5], Wp[5];
     weno_cell_states<T, DIR>(w, Wm, Wp);
+#ifdef JF_YZ_XCHG
+    T WmPrev[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { T* x = xw(q); WmPrev[q] = *x; *x = Wm[q]; }
+#endif
     // issue the loads this step consumes at its end
     const bool more = c < c1;                // another cell follows: its window needs padded pc+3
     const bool upd = c > c0;                 // cell c-1 is in [c0, c1): update it
@@ -666,18 +704,18 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     if (more) {
       const unsigned on = col + (unsigned)(pc + 3) * sm;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) raw[q] = (U + q * P.vol)[on];
+      for (int q = 0; q < 5; ++q) raw[q] = (MODE == 2) ? (U + q * P.vol)[on] : ld_stream((U + q * P.vol) + on);
       if (VISC) {
 #pragma unroll
-        for (int cc = 0; cc < 3; ++cc) gn[cc] = gsrc[cc][on];
+        for (int cc = 0; cc < 3; ++cc) gn[cc] = ld_stream(gsrc[cc] + on);
       }
     }
     if (upd) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) Rold[q] = (R + q * P.vol)[o];
+      for (int q = 0; q < 5; ++q) Rold[q] = ld_stream((R + q * P.vol) + o);
       if (MODE == 2) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) un[q] = (rk.Un + q * P.vol)[o];
+        for (int q = 0; q < 5; ++q) un[q] = ld_stream((rk.Un + q * P.vol) + o);
       }
     }
     if (c >= c0) {                           // face c-1/2
@@ -687,7 +725,11 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
         const T idl = idl_c;
         T Rv[5];
 #pragma unroll
+#ifdef JF_YZ_FSMEM
+        for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - fsm[q * NT]) * idl;
+#else
         for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - Fprev[q]) * idl;
+#endif
         if (MODE >= 1 && gas.has_g) {
           T rho = w(-1, 0), u = w(-1, 1), v = w(-1, 2), ww = w(-1, 3);
           Rv[1] += rho * gas.g[0]; Rv[2] += rho * gas.g[1]; Rv[3] += rho * gas.g[2];
@@ -697,19 +739,26 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
           // U_s of cell c-1 entered the window four steps ago: an L1/L2 hit, loaded where it is used
           // (loaded with the other arrays it costs the z sweep its last registers: spills)
 #pragma unroll
-          for (int q = 0; q < 5; ++q) us[q] = (U + q * P.vol)[o];
+          for (int q = 0; q < 5; ++q) us[q] = ld_last((U + q * P.vol) + o);
+          const T dtv = rk.dt_dev ? T(*rk.dt_dev) : rk.dt;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) (rk.Uout + q * P.vol)[o] = rk.a * un[q] + rk.b * (us[q] + rk.dt * Rv[q]);
+          for (int q = 0; q < 5; ++q) st_stream((rk.Uout + q * P.vol) + o, rk.a * un[q] + rk.b * (us[q] + dtv * Rv[q]));
         } else {
 #pragma unroll
-          for (int q = 0; q < 5; ++q) (R + q * P.vol)[o] = Rv[q];
+          for (int q = 0; q < 5; ++q) st_stream((R + q * P.vol) + o, Rv[q]);
         }
       }
 #pragma unroll
+#ifdef JF_YZ_FSMEM
+      for (int q = 0; q < 5; ++q) fsm[q * NT] = F[q];
+#else
       for (int q = 0; q < 5; ++q) Fprev[q] = F[q];
+#endif
     }
+#ifndef JF_YZ_XCHG
 #pragma unroll
     for (int q = 0; q < 5; ++q) WmPrev[q] = Wm[q];
+#endif
     if (more) put(s0, raw, gn);              // cell c+3 replaces cell c-2
     s0 = (s0 == YZ_RING - 1) ? 0 : s0 + 1;
   }
@@ -718,8 +767,13 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
 // ------------------------------------------------------------------ a8 CFL reduction
 // out[0..2] = min over interior cells of the three step limits (as ordered u64 bit patterns of
 // non-negative doubles), out[3] = inadmissible-state flag.
+// FIN (jf_cfl_dt_dev): the last block to finish forms the step on the device,
+//   dt = min(cfl * min(dt_conv, 3/14 dt_visc, 1/10 dt_heat), t_end - t),  out[5] = dt, out[6] = t + dt,
+// (NaN and out[7] = 1 if the flag is set), re-arms out[0..4] for the next reduction, and the z + RK sweep reads
+// out[5] directly (RKArgs::dt_dev): no host round trip between the reduction and the step.
 template <class T>
-__global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restrict__ U, unsigned long long* out) {
+__global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restrict__ U, unsigned long long* out, int fin,
+                                                  double cflnum, double t_end) {
   const Gas<T> gas = P.gas;
   const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
   T dconv = T(INFINITY), dvisc = T(INFINITY), dheat = T(INFINITY);
@@ -777,6 +831,26 @@ __global__ void __launch_bounds__(256) cfl_kernel(Params<T> P, const T* __restri
       atomicMin(&out[1], (unsigned long long)__double_as_longlong(b));
       atomicMin(&out[2], (unsigned long long)__double_as_longlong(c));
       if (bb) atomicOr(&out[3], 1ULL);
+      if (fin) {
+        __threadfence();
+        if (atomicAdd(&out[4], 1ULL) == (unsigned long long)gridDim.x - 1ULL) {   // every block has contributed
+          __threadfence();
+          const double dc = __longlong_as_double((long long)atomicAdd(&out[0], 0ULL));
+          const double dv = __longlong_as_double((long long)atomicAdd(&out[1], 0ULL));
+          const double dh = __longlong_as_double((long long)atomicAdd(&out[2], 0ULL));
+          const bool badst = atomicAdd(&out[3], 0ULL) != 0ULL;
+          double dt = dc;
+          if (gas.viscous) dt = fmin(dt, fmin((3.0 / 14.0) * dv, (1.0 / 10.0) * dh));
+          dt *= cflnum;
+          double* st = reinterpret_cast<double*>(out);
+          const double t = st[6];
+          if (t_end == t_end) dt = fmin(dt, t_end - t);        // t_end = NaN: no clipping
+          if (badst) { dt = __longlong_as_double(0x7ff8000000000000LL); out[7] = 1ULL; }
+          st[5] = dt;
+          st[6] = t + dt;
+          out[0] = out[1] = out[2] = ~0ULL; out[3] = 0ULL; out[4] = 0ULL;   // re-armed for the next call
+        }
+      }
     }
   }
 }

@@ -483,4 +483,73 @@ def test_abi_error_statuses(jf):
     n0 = s.jf_launch_count()
     s.jf_rk3_step(U, 1e-3)
     torch.cuda.synchronize()
-    assert s.jf_launch_count() - n0 == 3 * (1 + 4)
+    # 3 x (halo, gradient, x, y, z + RK) kernels, replayed from the solver's CUDA graph, plus the one-thread
+    # kernel that hands the host's dt to the graph
+    assert s.jf_launch_count() - n0 == 3 * (1 + 4) + 1
+
+
+# ------------------------------------------------------------------ CUDA graph replay and device-resident dt
+def _solver_without_graph(jf, c, dtype="f64"):
+    import os
+    old = os.environ.get("JF_GRAPH")
+    os.environ["JF_GRAPH"] = "0"
+    try:
+        return jf.Solver(c, dtype)
+    finally:
+        if old is None:
+            del os.environ["JF_GRAPH"]
+        else:
+            os.environ["JF_GRAPH"] = old
+
+
+@pytest.mark.parametrize("name", ["channel", "walls", "tgv_f32"])
+def test_graph_replay_is_bitwise_the_plain_launch_sequence(jf, name):
+    import torch
+    dtype = "f32" if name == "tgv_f32" else "f64"
+    c = {"channel": lambda: cases.channel(24, 16, 16), "walls": lambda: all_bc_case(n=(37, 21, 13), which=0),
+         "tgv_f32": lambda: cases.tgv(32)}[name]()
+    a, b = jf.Solver(c, dtype), _solver_without_graph(jf, c, dtype)
+    Ua, Ub = a.state(), b.state()
+    for k in range(4):
+        dt = 1e-3 * (1 + 0.1 * k)                            # a different dt every step: same graph
+        a.jf_rk3_step(Ua, dt)
+        b.jf_rk3_step(Ub, dt)
+    torch.cuda.synchronize()
+    assert b.jf_launch_count() == 4 * 15 and a.jf_launch_count() == 4 * 16
+    assert Ua.cpu().numpy().tobytes() == Ub.cpu().numpy().tobytes()
+    # a second state array gets its own graph
+    Va, Vb = a.state(), b.state()
+    a.jf_rk3_step(Va, 2e-3)
+    b.jf_rk3_step(Vb, 2e-3)
+    assert Va.cpu().numpy().tobytes() == Vb.cpu().numpy().tobytes()
+
+
+@pytest.mark.parametrize("name", ["channel", "sod", "plate"])
+def test_device_resident_dt_equals_the_host_loop(jf, ora, name):
+    # jf_cfl_dt_dev + jf_rk3_step_dev (the step is formed and consumed on the device, t_end clipping included)
+    # against jf_cfl_dt + jf_rk3_step: same dt sequence bit for bit, same state bit for bit; and against the oracle
+    c = {"channel": lambda: cases.channel(24, 16, 16, n_steps=12), "sod": lambda: cases.sod(64),
+         "plate": lambda: cases.flat_plate(64, 24, 8, n_steps=12)}[name]()
+    Uh, dth = jf.run_case(c, "f64")
+    Ud, dtd = jf.run_case(c, "f64", device_dt=True)
+    assert dth == dtd and len(dth) > 5
+    assert Uh.cpu().numpy().tobytes() == Ud.cpu().numpy().tobytes()
+    Uo, dto = ora.run_case(c, "f64")
+    assert len(dto) == len(dtd) and max(abs(x - y) / x for x, y in zip(dto, dtd)) <= 1e-12
+    assert np.all(metric_P(Ud.cpu().numpy(), Uo) <= TOL["f64"])
+
+
+def test_device_resident_dt_flags_bad_state(jf):
+    c = cases.random_admissible(n=(12, 10, 8), seed=1)
+    s = jf.Solver(c)
+    U = s.state()
+    s.jf_cfl_dt_dev(U, 0.5)
+    st, dt, t = s.jf_dev_time()
+    st_h, dt_h = s.jf_cfl_dt(U, 0.5)
+    assert st == jf.JF_OK and dt == dt_h and t == dt
+    U[0, NH + 1, NH + 2, NH + 3] = -1.0
+    s.jf_cfl_dt_dev(U, 0.5)
+    st, dt, t = s.jf_dev_time()
+    assert st == jf.JF_ENOTFINITE and np.isnan(dt)
+    st, dt, t = s.jf_dev_time(set_t=0.25)                     # reset clears the sticky status
+    assert st == jf.JF_OK and t == 0.25 and dt == 0.0
