@@ -40,6 +40,10 @@ def parse_args():
     ap.add_argument("--ref-size", type=int, default=96, help="n^3 sample the reference arm steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", dest="sweep", action="store_false",
+                    help="skip the other lines of configs[4] (384^3, 512^3 fp64, 512^3 fp32) the default run appends")
+    ap.add_argument("--decomp", default=None, metavar="Sx,Sy,Sz",
+                    help="block-decomposition arm: one --size^3 block per rank, Sx*Sy*Sz ranks (PAPER.md:78-82)")
     return ap.parse_args()
 
 
@@ -161,6 +165,60 @@ def job_throughput(cells_per_rank, steps, world, ms):
 
 
 # ---------------------------------------------------------------------------- our arm
+def measured_peaks():
+    ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    return json.load(open(ppath)) if os.path.exists(ppath) else {}
+
+
+def profile_row(kernel, n, dtype):
+    """Row of profiles/traffic.csv (hand-copied from the committed ncu --set full capture; profiles/traffic.md
+    names the command): DRAM bytes and executed FP64 thread-instructions per launch, averaged over the three
+    stage launches of one step.  None for sizes / dtypes without a row."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tpath):
+        return None
+    import csv
+    with open(tpath) as f:
+        for row in csv.DictReader(f):
+            if row["kernel"] == kernel and int(row["size"]) == n and row["dtype"] == dtype:
+                return row
+    return None
+
+
+def alu_peak(jf, dtype, local):
+    """Measured ALU peak (jf_diag_alu_peak: register-resident FMA loop).  burst: best of three short launches;
+    sustained: back to back for 1.5 s, median of the second half, with the SM clock sampled meanwhile."""
+    burst, _ = jf.jf_diag_alu_peak(dtype, 4096)
+    clk = ClockSampler(local)
+    clk.start()
+    samples, t_end = [], time.time() + 1.5
+    while time.time() < t_end or len(samples) < 8:
+        samples.append(jf.jf_diag_alu_peak(dtype, 4096)[0])
+    c = clk.stop()
+    tail = sorted(samples[len(samples) // 2:])
+    return burst, tail[len(tail) // 2], c.get("sm_mhz")
+
+
+def time_steps(torch, step, K, W, barrier, sampler=None):
+    for _ in range(W):
+        step()
+    barrier()
+    if sampler:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        step()
+    e1.record()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def t_roof_ms(flops_cell_step, cells, dtype, peak_flops, hbm_gbs):
+    """north_star: the slower of the path's FLOPs at the ALU peak and its algorithmic bytes at HBM bandwidth."""
+    return max(flops_cell_step * cells / peak_flops, (320 if dtype == "f64" else 160) * cells / (hbm_gbs * 1e9)) * 1e3
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -182,6 +240,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.decomp:
+        return run_decomp(args, torch, dist, jf, cases, world, rank, local, dev, barrier)
+
     n, K, W = args.size, args.steps, max(args.warmup, 3)
     channel = args.case == "channel"
     case = cases.channel() if channel else cases.tgv(n)
@@ -192,44 +253,29 @@ def run_ours(args):
     state_bytes = U.numel() * esz
 
     def step(V=None):
-        # fixed-dt configs (0, 4) time jf_rk3_step alone; CFL-driven configs (1-3) take jf_cfl_dt every step
+        # fixed-dt configs (0, 4) time jf_rk3_step alone; CFL-driven configs (1-3) take the CFL reduction every step,
+        # formed and consumed on the device (jf_cfl_dt_dev + jf_rk3_step_dev: no host round trip inside the loop)
         V = U if V is None else V
         if channel:
-            st, d = solver.jf_cfl_dt(V, case.cfl)
-            if st != 0:
-                raise SystemExit(f"bench.py: jf_cfl_dt status {st}")
-            solver.jf_rk3_step(V, d)
+            solver.jf_cfl_dt_dev(V, case.cfl)
+            solver.jf_rk3_step_dev(V)
         else:
             solver.jf_rk3_step(V, dt)
 
-    # --- device-resident throughput: inputs in HBM, K steps between two events
-    for _ in range(W):
-        step()
+    # --- device-resident throughput: inputs in HBM, K steps between two events, nothing else on the stream
     clocks = ClockSampler(local)
-    barrier()
-    clocks.start()
-    # timed region: K steps between two events, nothing else on the stream
+    step()                                             # first call captures the step's CUDA graph
     l0 = solver.jf_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(K):
-        step()
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = solver.jf_launch_count() - l0
-    # the same K steps once more with an event pair around every launch (jf_diag_timing): per-kernel durations for
-    # the roofline of the dominant kernel.  Kept out of the region above because the 30 extra event records per
-    # step cost 2 % at 256^3 and 10-40 % on the small boxes.
+    ms = time_steps(torch, step, K, W, barrier, clocks)
+    launches = (solver.jf_launch_count() - l0) * K // (K + W)
+    if channel and solver.jf_dev_time()[0] != 0:
+        raise SystemExit("bench.py: device-side CFL reduction flagged an inadmissible state")
+    # the same K steps once more with an event pair around every launch (jf_diag_timing; plain launches, no graph):
+    # per-kernel durations for the roofline of the dominant kernel.  Kept out of the region above because the 30
+    # extra event records per step cost 2 % at 256^3 and 10-40 % on the small boxes.
     solver.jf_diag_kernel_times()                      # reset
     solver.jf_diag_timing(True)
-    i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    i0.record()
-    for _ in range(K):
-        step()
-    i1.record()
-    barrier()
-    ms_instr = i0.elapsed_time(i1)
+    ms_instr = time_steps(torch, step, K, 0, barrier)
     ktimes = solver.jf_diag_kernel_times()
     solver.jf_diag_timing(False)
     clk = clocks.stop()
@@ -280,6 +326,28 @@ def run_ours(args):
         e2e = (ms_e2e, Ke)
         e2e_finite = bool(torch.isfinite(host_out[(Ke - 1) & 1]).all().item())
 
+    # --- the other lines of configs[4] (N = 1, default workload only): 384^3 and 512^3 fp64, 512^3 fp32
+    sweep = None
+    if world == 1 and not channel and args.sweep and n == 256 and args.dtype == "f64":
+        del solver, U
+        if e2e:
+            del bufs, host_in, host_out
+        torch.cuda.empty_cache()
+        sweep = []
+        for sn, sdt in ((384, "f64"), (512, "f64"), (512, "f32")):
+            sc = cases.tgv(sn)
+            ss = jf.Solver(sc, sdt, device=str(dev))
+            SU = ss.state()
+            sck = ClockSampler(local)
+            ss.jf_rk3_step(SU, sc.dt)
+            sms = time_steps(torch, lambda: ss.jf_rk3_step(SU, sc.dt), 5, 3, barrier, sck)
+            sclk = sck.stop()
+            sweep.append({"size": sn, "dtype": sdt, "cells": sc.cells, "steps": 5, "ms_per_step": sms / 5,
+                          "value": sc.cells * 5 / (sms * 1e-3), "sm_mhz": sclk.get("sm_mhz"), "reasons": sclk.get("reasons"),
+                          "finite": bool(torch.isfinite(SU).all().item())})
+            del ss, SU
+            torch.cuda.empty_cache()
+
     # --- max over ranks
     if world > 1:
         ms, e2e_ms = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, dev)
@@ -296,16 +364,13 @@ def run_ours(args):
         with open(os.path.join(ROOT, "oracle", "flop_model.json")) as f:
             ch = json.load(f)["channel_step"][3]
         fm = {k: v * ch / fm["step"] for k, v in fm.items()}   # pieces scaled like the Taylor-Green split
-    # roofline of the dominant kernel (bound: plain FP64/FP32 ALUs; nothing here is a contraction)
-    # burst: best of three short launches; sustained: the same loop launched back to back for >= 1.5 s, median of
-    # the second half (the clocks settle where a long run holds them).  The step kernels are timed inside a long
-    # run, so the sustained figure is the roofline's peak; the burst figure is reported beside it.
-    peak_burst, _ = jf.jf_diag_alu_peak(args.dtype, 4096)
-    samples, t_end = [], time.time() + 1.5
-    while time.time() < t_end or len(samples) < 8:
-        samples.append(jf.jf_diag_alu_peak(args.dtype, 4096)[0])
-    tail = sorted(samples[len(samples) // 2:])
-    peak_flops = tail[len(tail) // 2]
+    # roofline of the dominant kernel (bound: plain FP64/FP32 ALUs; nothing here is a contraction).  The step kernels
+    # are timed inside a long run, so the sustained peak is the roofline's; the burst figure is reported beside it.
+    # The peak loop holds the maximum SM clock while the step runs into the board's power cap, so the fraction at the
+    # clock the step actually ran at is reported too (peak scaled by run clock / peak-loop clock).
+    peak_burst, peak_flops, peak_mhz = alu_peak(jf, args.dtype, local)
+    run_mhz = clk.get("sm_mhz")
+    clock_ratio = (run_mhz / peak_mhz) if (run_mhz and peak_mhz) else None
     sweep_flops = (fm["rhs"] - fm["prim"] - fm["grad"]) / 3.0           # one direction: WENO5+HLLC+viscous face+divergence
     rk_flops = (fm["step"] - 3.0 * fm["rhs"]) / 3.0                    # stage update
     alg = {"sweep_x_kernel": sweep_flops + fm["prim"] / 3.0, "sweep_yz_kernel<y>": sweep_flops + fm["prim"] / 3.0,
@@ -313,45 +378,57 @@ def run_ours(args):
     dom = max((k for k in ktimes if ktimes[k][1] > 0), key=lambda k: ktimes[k][0])
     dom_ms, dom_n = ktimes[dom]
     dom_flops = alg.get(dom, 0.0) * cells
-    achieved = dom_flops / (dom_ms / dom_n * 1e-3) / 1e12 if dom_n else 0.0
-    # measured DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of the
-    # committed ncu --set full capture; profiles/traffic.csv names its source), null if not captured for this size
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tpath):
-        import csv
-        with open(tpath) as f:
-            for row in csv.DictReader(f):
-                if not channel and row["kernel"] == dom and int(row["size"]) == n and row["dtype"] == args.dtype:
-                    traffic = float(row["dram_bytes_per_launch"])
-    peaks = {}
-    ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(ppath):
-        peaks = json.load(open(ppath))
+    dom_s = dom_ms / dom_n * 1e-3 if dom_n else None
+    achieved = dom_flops / dom_s / 1e12 if dom_n else 0.0
+    # measured DRAM bytes and executed FP64 instructions of the dominant kernel (committed ncu capture)
+    row = None if channel else profile_row(dom, n, args.dtype)
+    traffic = float(row["dram_bytes_per_launch"]) if row else None
+    executed = None
+    if row and row.get("dfma_thread_inst"):
+        ex_flops = 2.0 * float(row["dfma_thread_inst"]) + float(row["dadd_thread_inst"]) + float(row["dmul_thread_inst"])
+        executed = {"flops_per_launch": ex_flops, "achieved": ex_flops / dom_s / 1e12, "frac": ex_flops / dom_s / peak_flops,
+                    "numerator": "2*DFMA + DADD + DMUL thread-instructions of the launch (ncu smsp__sass_thread_inst_executed_op_*; "
+                                 "divisions / square roots appear as the Newton steps they are executed as)"}
+    peaks = measured_peaks()
     hbm = peaks.get("hbm_gbs", 6650.0)
-    t_roof_ms = max(fm["step"] * cells / peak_flops, (320 if args.dtype == "f64" else 160) * cells / (hbm * 1e9)) * 1e3
+    troof = t_roof_ms(fm["step"], cells, args.dtype, peak_flops, hbm)
+    if sweep:
+        for ln in sweep:
+            sfm = flop_model(ln["size"])
+            pk = peak_flops if ln["dtype"] == args.dtype else alu_peak(jf, ln["dtype"], local)[1]
+            tr = t_roof_ms(sfm["step"], ln["cells"], ln["dtype"], pk, hbm)
+            ln["roofline_step_frac"] = tr / ln["ms_per_step"]
+            ln["peak_tflops"] = pk / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "ms_per_step_with_per_launch_events": ms_instr / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": ("channel 192x128x128 (BASELINE.json configs[2]: isothermal walls, Sutherland, body force, tanh y grid; "
-                                "jf_cfl_dt + jf_rk3_step every step)") if channel else
+                                "jf_cfl_dt_dev + jf_rk3_step_dev every step)") if channel else
                                f"tgv{n} {'fp64' if args.dtype == 'f64' else 'fp32'} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)",
                    "cells": cells, "state_bytes": state_bytes, "l2": "inputs larger than L2 (no flush)" if state_bytes > 126e6 else "state fits L2",
-                   "parallelism": f"replicas x{world}" if world > 1 else "1 GPU", "finite": finite},
+                   "parallelism": f"replicas x{world}" if world > 1 else "1 GPU", "finite": finite,
+                   "launch": "CUDA graph of the 15 kernels of a step, replayed (+ 1 one-thread kernel carrying a host dt)"},
         "clocks": clk,
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
                      "frac": achieved / (peak_flops / 1e12), "traffic": traffic,
+                     "numerator": "algorithmic flops: the oracle's own operation count (add/sub/mul/min/max/div/sqrt = 1), oracle/flop_model.json",
+                     "frac_at_run_clock": achieved / (peak_flops / 1e12) / clock_ratio if clock_ratio else None,
+                     "peak_loop_sm_mhz": peak_mhz, "run_sm_mhz": run_mhz,
+                     "executed": executed,
                      "peak_burst": peak_burst / 1e12, "frac_of_burst": achieved / (peak_burst / 1e12),
                      "peak_source": "measured live, sustained: jf_diag_alu_peak register-resident FMA loop back to back for 1.5 s (DESIGN.md)",
                      "flops_per_cell_launch": alg.get(dom), "avg_launch_ms": dom_ms / dom_n if dom_n else None},
-        "roofline_step": {"flops_per_cell_step": fm["step"], "t_roof_ms": t_roof_ms, "frac": t_roof_ms / (ms / K),
-                          "frac_of_burst_peak": max(fm["step"] * cells / peak_burst, (320 if args.dtype == "f64" else 160) * cells / (hbm * 1e9)) * 1e3 / (ms / K),
+        "roofline_step": {"flops_per_cell_step": fm["step"], "t_roof_ms": troof, "frac": troof / (ms / K),
+                          "frac_at_run_clock": troof / (ms / K) / clock_ratio if clock_ratio else None,
+                          "frac_of_burst_peak": t_roof_ms(fm["step"], cells, args.dtype, peak_burst, hbm) / (ms / K),
                           "hbm_gbs": hbm, "hbm_source": "measured" if peaks else "fallback"},
         "kernels_ms_per_step": {k: v[0] / K for k, v in ktimes.items() if v[1]},
     }
+    if sweep:
+        line["sweep"] = sweep
     if e2e:
         line["e2e"] = {"value": job_throughput(cells, e2e[1], world, e2e[0]), "unit": UNIT,
                        "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes, "ms_per_step": e2e[0] / e2e[1],
@@ -364,6 +441,47 @@ def run_ours(args):
                                 "sample": (f"1 step (cfl_dt + RK3) of the channel 192x128x128 fp64 ({secs:.1f} s)" if channel
                                            else f"1 RK3 step of tgv{nb} fp64 ({secs:.1f} s)")}
     print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------- block decomposition arm
+def pid_seconds(ms_per_step, ranks, dof):
+    """The paper's performance index, Eq. 9: PID = wall time per step x #ranks / #DOF."""
+    return ms_per_step * 1e-3 * ranks / dof
+
+
+def run_decomp(args, torch, dist, jf, cases, world, rank, local, dev, barrier):
+    """--decomp Sx,Sy,Sz: the paper's own parallel strategy, one n^3 Taylor-Green block per rank
+    (weak scaling), halos of inter-block faces exchanged point-to-point three times per RK stage (decomp.RankBlock).
+    Needs Sx*Sy*Sz ranks.  Prints cell-updates/s of the whole job and the PID of Eq. 9 next to it."""
+    from paper_2406_19494_b200 import decomp
+    S = tuple(int(v) for v in args.decomp.split(","))
+    if len(S) != 3 or S[0] * S[1] * S[2] != world:
+        raise SystemExit(f"bench.py --decomp {args.decomp}: needs {S[0] * S[1] * S[2] if len(S) == 3 else '?'} ranks, have {world}")
+    n, K, W = args.size, args.steps, max(args.warmup, 3)
+    part = decomp.tgv_part(n, S, rank)
+    rb = decomp.RankBlock(None, S, args.dtype, device=str(dev), part=part)
+    dt = part.case.dt
+    clocks = ClockSampler(local)
+    ms = time_steps(torch, lambda: rb.jf_rk3_step(dt), K, W, barrier, clocks)
+    clk = clocks.stop()
+    finite = bool(torch.isfinite(rb.U).all().item())
+    (ms,) = max_over_ranks([ms], world, dev)
+    if rank == 0:
+        cells = part.case.cells
+        line = {"metric": METRIC, "value": job_throughput(cells, K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": args.dtype, "data": "synthetic",
+                "config": {"workload": f"tgv {n}^3 per rank, blocks {S[0]}x{S[1]}x{S[2]} (PAPER.md:78-82 decomposition; global "
+                                       f"{n * S[0]}x{n * S[1]}x{n * S[2]})", "cells_per_rank": cells, "finite": finite,
+                           "parallelism": f"domain decomposition {S[0]}x{S[1]}x{S[2]}, halo exchange by NCCL point-to-point",
+                           "exchange_bytes_per_rank_per_step": rb.exchange_bytes_per_step()},
+                "clocks": clk, "gpu_launches": int(rb.solver.jf_launch_count() * K // (K + W)),
+                "pid": {"eq": "PAPER.md:130 Eq. 9: wall time per step x ranks / DOF",
+                        "dof_cells": pid_seconds(ms / K, world, cells * world),
+                        "dof_cells_x5": pid_seconds(ms / K, world, 5 * cells * world), "unit": "s"}}
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 

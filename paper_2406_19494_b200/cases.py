@@ -82,12 +82,24 @@ def periodic_bc():
 
 
 # ------------------------------------------------------------------ config 0 / 4: Taylor-Green
-def tgv(n=32, dt=1e-3, n_steps=10):
+def tgv(n=32, dt=1e-3, n_steps=10, faces=None):
     """Taylor-Green vortex, periodic [0,2pi]^3, gamma=1.4, Pr=0.71, M=0.1, Re=1600, constant mu
-    (BASELINE.json configs[0], configs[4])."""
+    (BASELINE.json configs[0], configs[4]).  faces = (xf, yf, zf): the same field on another
+    box (the field has period 2 pi along every axis: a block of a [0, 2 pi S]^3 box for the decomposition bench)."""
     gamma, M, Re = 1.4, 0.1, 1600.0
     p0 = 1.0 / (gamma * M * M)
     R = p0                       # rho0 = T0 = 1
+    if faces is not None:
+        fx, fy, fz = (np.asarray(a, dtype=np.float64) for a in faces)
+        nn = (len(fx) - 1, len(fy) - 1, len(fz) - 1)
+        Z, Y, X = np.meshgrid(centres(fz), centres(fy), centres(fx), indexing="ij")
+        u = np.sin(X) * np.cos(Y) * np.cos(Z)
+        v = -np.cos(X) * np.sin(Y) * np.cos(Z)
+        p = p0 + (1.0 / 16.0) * (np.cos(2 * X) + np.cos(2 * Y)) * (np.cos(2 * Z) + 2.0)
+        U = set_interior_from_prim(empty_state(nn), gamma, p / R, u, v, np.zeros_like(u), p)
+        return Case(name=f"tgv{nn[0]}x{nn[1]}x{nn[2]}", n=nn, xf=fx, yf=fy, zf=fz, gamma=gamma, R_gas=R,
+                    Pr=0.71, mu={"sutherland": 0, "mu_ref": 1.0 / Re, "T_ref": 1.0, "S": 0.0},
+                    bc=periodic_bc(), U0=U, dt=dt, n_steps=n_steps)
     f = uniform_faces(0.0, 2.0 * np.pi, n)
     c = centres(f)
     Z, Y, X = np.meshgrid(c, c, c, indexing="ij")

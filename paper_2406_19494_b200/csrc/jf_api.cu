@@ -797,7 +797,7 @@ jf_status jf_diag_kernel_times(jf_solver* s, double ms[6], unsigned long long la
 }
 
 const char* jf_diag_kernel_name(int k) {
-  static const char* names[K_COUNT] = {"halo_kernel", "gradient_kernel", "sweep_x_kernel", "sweep_yz_kernel<y>",
+  static const char* names[K_COUNT] = {"halo_all_kernel", "gradient_kernel", "sweep_x_kernel", "sweep_yz_kernel<y>",
                                        "sweep_yz_kernel<z>+rk", "cfl_kernel"};
   return (k >= 0 && k < K_COUNT) ? names[k] : "";
 }

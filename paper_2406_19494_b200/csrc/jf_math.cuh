@@ -177,7 +177,8 @@ __device__ __forceinline__ T viscosity(const Gas<T>& gas, T Tf) {
 //   first-derivative parts of the indicators  a-4b+3c = A0+2 D2,  b-d = -(D2+D3),  3c-4d+e = A2-2 D3;
 //   candidates  p1 = c + D3/3 + D2/6,  p0-p1 = (A0-A1)/3,  p2-p1 = (A1-A2)/6  (mirrored: p1' = c - D2/3 - D3/6).
 // v = p1 + [w0 (p0-p1) + w2 (p2-p1)] / sum with the weights as products of the other two
-// e_k = (beta_k+eps)^2 (one reciprocal per value); with t1 = E12 (A0-A1), t2 = E01 (A1-A2):
+// e_k = (beta_k+eps)^2 (one reciprocal per value; fp32 forms 1/e_k instead, see below); with t1 = E12 (A0-A1),
+// t2 = E01 (A1-A2):
 //   vm = c + D2/6 + [D3 + (t1 + 1.5 t2)/(E12 + 6 E02 + 3 E01)]/3,
 //   vp = c - D3/6 - [D2 + (1.5 t1 + t2)/(3 E12 + 6 E02 + E01)]/3.
 // Indicators are carried as 4*beta (eps scaled likewise), which leaves the weights unchanged.
@@ -192,8 +193,17 @@ __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp
   T e0 = N::fma_(c133 * A0, A0, N::fma_(b0, b0, eps4));
   T e1 = N::fma_(c133 * A1, A1, N::fma_(b1, b1, eps4));
   T e2 = N::fma_(c133 * A2, A2, N::fma_(b2, b2, eps4));
-  e0 *= e0; e1 *= e1; e2 *= e2;
-  T E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
+  T E12, E02, E01;
+  if (sizeof(T) == 4) {
+    // fp32: the pair products e_k e_l ~ beta^4 ~ (jump)^8 leave the exponent range once a primitive jumps by ~1e4
+    // (SI pressures with a mild shock).  Dividing all three products by e_0 e_1 e_2 leaves the weights unchanged
+    // and gives (E12, E02, E01) = (1/e_0, 1/e_1, 1/e_2): three reciprocals, every factor within range.
+    const T r0 = N::rcp(e0), r1 = N::rcp(e1), r2 = N::rcp(e2);
+    E12 = r0 * r0; E02 = r1 * r1; E01 = r2 * r2;
+  } else {
+    e0 *= e0; e1 *= e1; e2 *= e2;
+    E12 = e1 * e2; E02 = e0 * e2; E01 = e0 * e1;
+  }
   T t1 = E12 * (A0 - A1), t2 = E01 * (A1 - A2);
   {  // face i+1/2: weights (0.1 E12, 0.6 E02, 0.3 E01)
     T den = N::fma_(T(3), E01, N::fma_(T(6), E02, E12));

@@ -104,6 +104,49 @@ def split_case(case, blocks):
     return parts
 
 
+def exchange_faces(case_bc, S, b, lo, hi, faces, widths, N):
+    """Face BCs and neighbour ranks of block b = (bx, by, bz) of an S[0] x S[1] x S[2] cut: physical faces keep the
+    case's BC (returned as None here: the caller copies it), faces between blocks become BC_EXCHANGE carrying the
+    neighbour's geometry (face coordinates across an interior cut, cell widths across a periodic wrap)."""
+    rank_of = lambda c: (c[2] * S[1] + c[1]) * S[0] + c[0]
+    bcs, nbs = [], []
+    for f in range(6):
+        a, side = f // 2, f % 2
+        at_edge = b[a] == (0 if side == 0 else S[a] - 1)
+        if at_edge and (case_bc[f].type != cases.BC_PERIODIC or S[a] == 1):
+            bcs.append(None)
+            nbs.append(None)
+            continue
+        nb = list(b)
+        nb[a] = (b[a] + (-1 if side == 0 else 1)) % S[a]
+        idx = [(lo[a] - m) % N[a] for m in (1, 2, 3)] if side == 0 else [(hi[a] + m) % N[a] for m in (0, 1, 2)]
+        nbf = None
+        if not at_edge:
+            nbf = tuple(float(faces[a][lo[a] - m]) for m in (1, 2, 3)) if side == 0 else \
+                tuple(float(faces[a][hi[a] + m]) for m in (1, 2, 3))
+        bcs.append(cases.FaceBC(cases.BC_EXCHANGE, nb_width=tuple(float(widths[a][i]) for i in idx), nb_face=nbf))
+        nbs.append(rank_of(nb))
+    return bcs, nbs
+
+
+def tgv_part(n, S, rank):
+    """Block `rank` of the weak-scaling decomposition bench: the Taylor-Green field (period 2 pi) on the box
+    [0, 2 pi S[0]] x [0, 2 pi S[1]] x [0, 2 pi S[2]] cut into S[0] x S[1] x S[2] blocks of n^3 cells.  Only this
+    rank's block is materialised (a 512^3 global state per rank would not be)."""
+    S = tuple(int(v) for v in S)
+    b = (rank % S[0], (rank // S[0]) % S[1], rank // (S[0] * S[1]))
+    N = [n * S[a] for a in range(3)]
+    faces = [cases.uniform_faces(0.0, 2.0 * np.pi * S[a], N[a]) for a in range(3)]
+    widths = [np.diff(f) for f in faces]
+    lo = [b[a] * n for a in range(3)]
+    hi = [lo[a] + n for a in range(3)]
+    sub = cases.tgv(n, faces=tuple(faces[a][lo[a]:hi[a] + 1].copy() for a in range(3)))
+    bcs, nbs = exchange_faces(cases.periodic_bc(), S, b, lo, hi, faces, widths, N)
+    sub.bc = [cases.FaceBC(cases.BC_PERIODIC) if x is None else x for x in bcs]
+    sub.name = f"tgv{n}@{b[0]}.{b[1]}.{b[2]}of{S[0]}x{S[1]}x{S[2]}"
+    return Part(sub, b, tuple(lo), nbs)
+
+
 def gather_interior(case, parts, arrays):
     """Global padded array (halos zero) from the blocks' arrays [5, nz+6, ny+6, nx+6(, 2)]."""
     extra = arrays[0].shape[4:]
@@ -117,8 +160,8 @@ def gather_interior(case, parts, arrays):
 
 
 class MultiBlock:
-    """All blocks of a decomposed case driven from one process (their arrays on one device, or on several
-    devices of one node with peer access enabled): inter-block halos by `jf_pull_face`."""
+    """All blocks of a decomposed case driven from one process, their arrays on ONE device (all launches on that
+    device's current stream, which orders the blocks): inter-block halos by `jf_pull_face`, or pack -> unpack."""
 
     def __init__(self, case, blocks, dtype="f64", device="cuda:0", transport="pull"):
         from . import binding
@@ -126,6 +169,7 @@ class MultiBlock:
         self.case, self.parts, self.transport = case, split_case(case, blocks), transport
         self.solvers = [binding.Solver(p.case, dtype, device) for p in self.parts]
         self.U = [s.state() for s in self.solvers]
+        self._bufs = {}
 
     def fill_halos(self, ptrs):
         """Halo fill of the arrays at raw device pointers ptrs[rank], axis by axis (include/jf.h)."""
@@ -142,8 +186,11 @@ class MultiBlock:
                         s.jf_pull_face(ptrs[r], f, ptrs[nb], self.parts[nb].case.n)
                     else:                                # what the neighbour packs for its opposite face
                         sn = self.solvers[nb]
-                        buf = sn.torch.empty(sn.jf_face_elems(f ^ 1) * (2 if sn.dtype == "f64t" else 1),
-                                             dtype=sn.tdtype, device=sn.device)
+                        key = (nb, f ^ 1)
+                        if key not in self._bufs:
+                            self._bufs[key] = sn.torch.empty(sn.jf_face_elems(f ^ 1) * (2 if sn.dtype == "f64t" else 1),
+                                                             dtype=sn.tdtype, device=sn.device)
+                        buf = self._bufs[key]
                         sn.jf_pack_face(ptrs[nb], f ^ 1, buf)
                         s.jf_unpack_face(ptrs[r], f, buf)
 
@@ -205,26 +252,43 @@ def exchange_axis(axis, neighbours, rank, pack, unpack, new_buffer, dist):
 
 class RankBlock:
     """This rank's block of a decomposed case (one process per GPU; `torch.distributed` initialised by the
-    caller, backend nccl): halos of inter-block faces by `jf_pack_face` -> point-to-point -> `jf_unpack_face`."""
+    caller, backend nccl): halos of inter-block faces by `jf_pack_face` -> point-to-point -> `jf_unpack_face`.
+    The send / receive buffers of the six faces are allocated once.  Not measured on hardware: this environment
+    has one GPU."""
 
-    def __init__(self, case, blocks, dtype="f64", device=None):
+    def __init__(self, case, blocks, dtype="f64", device=None, part=None):
         import torch
         import torch.distributed as dist
         from . import binding
         self.torch, self.dist = torch, dist
         self.rank, world = dist.get_rank(), dist.get_world_size()
-        self.parts = split_case(case, blocks)
-        if len(self.parts) != world:
-            raise ValueError(f"{len(self.parts)} blocks for {world} ranks")
-        self.part = self.parts[self.rank]
+        if part is None:
+            parts = split_case(case, blocks)
+            if len(parts) != world:
+                raise ValueError(f"{len(parts)} blocks for {world} ranks")
+            part = parts[self.rank]
+        self.part = part
         device = device or f"cuda:{torch.cuda.current_device()}"
         self.solver = binding.Solver(self.part.case, dtype, device)
         self.U = self.solver.state()
         self._bufs = {}
+        self._turn = {}
 
     def _new_buffer(self, face):
-        n = self.solver.jf_face_elems(face) * (2 if self.solver.dtype == "f64t" else 1)
-        return self.torch.empty(n, dtype=self.solver.tdtype, device=self.solver.device)
+        # two persistent buffers per face, handed out alternately: exchange_axis asks for the send buffer of a
+        # face first and for its receive buffer second
+        if face not in self._bufs:
+            n = self.solver.jf_face_elems(face) * (2 if self.solver.dtype == "f64t" else 1)
+            self._bufs[face] = [self.torch.empty(n, dtype=self.solver.tdtype, device=self.solver.device) for _ in range(2)]
+            self._turn[face] = 0
+        b = self._bufs[face][self._turn[face]]
+        self._turn[face] ^= 1
+        return b
+
+    def exchange_bytes_per_step(self):
+        """Bytes this rank sends per RK3 step: 3 stages x its exchange faces x 3 layers x 5 variables."""
+        esz = {"f64": 8, "f32": 4, "f64t": 16}[self.solver.dtype]
+        return 3 * sum(self.solver.jf_face_elems(f) * esz for f in range(6) if self.part.neighbours[f] is not None)
 
     def fill_halos(self, ptr):
         s = self.solver
@@ -240,6 +304,14 @@ class RankBlock:
 
     def jf_cfl_dt(self, cfl):
         st, dt = self.solver.jf_cfl_dt(self.U, cfl)
-        t = self.torch.tensor([dt if st == 0 else float("nan")], dtype=self.torch.float64, device=self.solver.device)
-        self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
-        return st, float(t[0])
+        return reduce_dt(st, dt, self.torch, self.dist, self.solver.device)
+
+
+def reduce_dt(st, dt, torch, dist, device=None):
+    """All ranks get the same (status, dt): status = MAX over ranks, dt = MIN over ranks with +inf standing in for a
+    rank whose reduction flagged an inadmissible state (a NaN fed to a MIN all-reduce is not reliably propagated);
+    dt is NaN whenever the status is not 0, so that no rank steps on while another has failed."""
+    t = torch.tensor([float("inf") if st != 0 else dt, -float(st)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    st_all = int(round(-float(t[1])))
+    return st_all, (float("nan") if st_all != 0 else float(t[0]))

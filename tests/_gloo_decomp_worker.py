@@ -73,8 +73,20 @@ exp = G[:, ix[2]][:, :, ix[1]][:, :, :, ix[0]]
 ok = bool(np.array_equal(U, exp))
 res = torch.tensor([1.0 if ok else 0.0])
 dist.all_reduce(res, op=dist.ReduceOp.MIN)
-t = torch.tensor([0.5 + rank], dtype=torch.float64)            # the dt all-reduce of RankBlock.jf_cfl_dt
-dist.all_reduce(t, op=dist.ReduceOp.MIN)
+# the (status, dt) reduction of RankBlock.jf_cfl_dt: MIN of dt, and a failed rank fails every rank with dt = NaN
+st_ok, dt_ok = decomp.reduce_dt(0, 0.5 + rank, torch, dist)
+st_bad, dt_bad = decomp.reduce_dt(5 if rank == 1 else 0, float("nan") if rank == 1 else 0.25, torch, dist)
+flags = torch.tensor([1.0 if (st_ok == 0 and dt_ok == 0.5 and st_bad == 5 and dt_bad != dt_bad) else 0.0])
+dist.all_reduce(flags, op=dist.ReduceOp.MIN)                   # ... on EVERY rank
+# the bench arm's own block: tgv_part materialises this rank's block only and must equal the cut of the global case
+tp = decomp.tgv_part(8, blocks, rank)
+g = cases.tgv(8, faces=tuple(cases.uniform_faces(0.0, 2.0 * np.pi * s, 8 * s) for s in blocks))
+gp = decomp.split_case(g, blocks)[rank]
+same = np.array_equal(tp.case.U0, gp.case.U0) and tp.neighbours == gp.neighbours and tp.lo == gp.lo and all(
+    a.type == b.type and a.nb_width == b.nb_width and a.nb_face == b.nb_face for a, b in zip(tp.case.bc, gp.case.bc))
+flags2 = torch.tensor([1.0 if same else 0.0])
+dist.all_reduce(flags2, op=dist.ReduceOp.MIN)
 if rank == 0:
-    print(json.dumps({"all_ranks_match": bool(res.item() == 1.0), "dt_min": float(t[0]), "blocks": blocks}), flush=True)
+    print(json.dumps({"all_ranks_match": bool(res.item() == 1.0), "dt_min": dt_ok, "status_reduction_ok": bool(flags.item() == 1.0),
+                      "tgv_part_ok": bool(flags2.item() == 1.0), "blocks": blocks}), flush=True)
 dist.destroy_process_group()

@@ -62,3 +62,21 @@ def test_two_rank_gloo_halo_exchange(blocks):
     assert out.returncode == 0, out.stderr[-3000:]
     d = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
     assert d["all_ranks_match"] is True and d["dt_min"] == 0.5
+    assert d["status_reduction_ok"] is True and d["tgv_part_ok"] is True
+
+
+def test_interior_cuts_carry_the_neighbours_face_coordinates():
+    # across an interior cut the halo cells take widths and centres from the neighbour's FACES (the undivided grid's
+    # own expressions); across a periodic wrap from its cell widths (which is what the undivided grid does there)
+    c = cases.channel(24, 16, 8, n_steps=1)
+    parts = decomp.split_case(c, (2, 2, 1))
+    p00, p01 = parts[0], parts[2]
+    assert p00.case.bc[3].nb_face == tuple(c.yf[9:12]) and p01.case.bc[2].nb_face == tuple(c.yf[7:4:-1])
+    assert p00.case.bc[0].nb_face is None and p00.case.bc[1].nb_face == tuple(c.xf[13:16])   # x-: wrap, x+: interior cut
+
+
+def test_pid_is_equation_9():
+    sys.path.insert(0, ROOT)
+    import bench
+    # PAPER.md:130 Eq. 9: wall time x ranks / DOF; the paper's own figures: < 0.1 s per step on 8 GPUs for 4.2 M cells
+    assert bench.pid_seconds(100.0, 8, 256 * 128 * 128) == pytest.approx(0.1 * 8 / 4194304)

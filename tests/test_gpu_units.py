@@ -71,6 +71,34 @@ def test_face_flux_matches_oracle_functions(jf, ora, d, kind):
     assert np.max(np.abs(F32 - Fo) / scale) <= 1e-4
 
 
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_fp32_face_flux_in_si_units_with_strong_jumps(jf, ora, d):
+    # fp32 with dimensional data: p ~ 1e5 Pa, rho ~ 1 kg/m3, u ~ 300 m/s and jumps of 1e4 .. 1e5 Pa inside the
+    # stencil.  Weights formed from products of (beta+eps)^2 overflow here (beta ~ jump^2 => product ~ jump^8);
+    # the fp32 kernels form them from reciprocals and must stay finite and within fp32 accuracy of the oracle.
+    rng = np.random.default_rng(40 + d)
+    n = 400
+    W = np.empty((n, 6, 6))
+    W[:, :, 0] = rng.uniform(0.8, 1.3, (n, 1)) + 0.05 * rng.uniform(-1, 1, (n, 6))
+    W[:, :, 1:4] = rng.uniform(-300, 300, (n, 1, 3)) + 20.0 * rng.uniform(-1, 1, (n, 6, 3))
+    W[:, :, 4] = rng.uniform(0.9e5, 1.1e5, (n, 1)) + 500.0 * rng.uniform(-1, 1, (n, 6))
+    k = rng.integers(1, 6, n)
+    jump = rng.uniform(1e4, 1e5, n) * rng.choice([-0.5, 1.0], n)     # never below ~4e4 Pa
+    for f in range(n):
+        W[f, k[f]:, 4] += jump[f]
+        W[f, k[f]:, 0] *= 1.0 + 0.5 * jump[f] / 1e5
+    Rg = 287.058
+    W[:, :, 5] = W[:, :, 4] / (W[:, :, 0] * Rg)
+    mu = {"sutherland": 0, "mu_ref": 0.0, "T_ref": 1.0, "S": 0.0}
+    F32 = jf.jf_diag_face_flux("f32", d, G, Rg, PR, mu, W)
+    assert np.isfinite(F32).all()
+    Fo = np.array([oracle_face(ora, d, W[f], None, 1.0, mu) for f in range(n)])
+    scale = np.max(np.abs(Fo), axis=1, keepdims=True)
+    assert np.max(np.abs(F32 - Fo) / scale) <= 1e-4
+    F64 = jf.jf_diag_face_flux("f64", d, G, Rg, PR, mu, W)
+    assert np.max(np.abs(F64 - Fo) / scale) <= 5e-14
+
+
 def test_face_flux_consistency_on_uniform_stencils(jf, ora):
     # F(W,W) = F^c(W) (Eq. 3) to round-off on the GPU as well
     rng = np.random.default_rng(3)
