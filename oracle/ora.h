@@ -56,6 +56,9 @@ typedef struct { ora_bc_face face[6]; } ora_bc; /* x-, x+, y-, y+, z-, z+ */
 /* --- the five calls (same meaning as include/jf.h, on host arrays) --- */
 int ora_create(ora_solver **out, const ora_grid *g, int dtype, double gamma, double R_gas,
                double Pr, const ora_mu_law *mu, const ora_bc *bc, const double body_accel[3]);
+/* order of the central dissipative-flux stencils: 4 (default; north_star) or 6:
+   centre / face derivatives, face interpolation and the index-space metrics all switch together */
+int ora_set_visc_order(ora_solver *s, int order);
 void ora_destroy(ora_solver *s);
 size_t ora_state_elems(const ora_solver *s);
 int ora_fill_halo(ora_solver *s, void *U);
@@ -98,6 +101,10 @@ double ora_viscosity(const ora_mu_law *mu, double T);
 double ora_dc(const double phi[5], double Xc);  /* phi[0..4] = i-2..i+2 */
 double ora_df(const double phi[4], double Xf);  /* phi[0..3] = i-1..i+2, face i+1/2 */
 double ora_if(const double phi[4]);
+/* sixth-order members: phi[0..6] = i-3..i+3 (centre), phi[0..5] = i-2..i+3 (face i+1/2) */
+double ora_dc6(const double phi[7], double Xc);
+double ora_df6(const double phi[6], double Xf);
+double ora_if6(const double phi[6]);
 /* dissipative flux of one face (dir, face index (i,j,k) = the cell on its low side) */
 int ora_viscous_face(ora_solver *s, const void *U, int dir, int i, int j, int k, double Fd[5]);
 

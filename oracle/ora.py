@@ -91,6 +91,13 @@ def lib(variant="ref"):
         L.ora_df.restype = C.c_double
         L.ora_if.argtypes = [c_double_p]
         L.ora_if.restype = C.c_double
+        L.ora_set_visc_order.argtypes = [C.c_void_p, C.c_int]
+        L.ora_dc6.argtypes = [c_double_p, C.c_double]
+        L.ora_dc6.restype = C.c_double
+        L.ora_df6.argtypes = [c_double_p, C.c_double]
+        L.ora_df6.restype = C.c_double
+        L.ora_if6.argtypes = [c_double_p]
+        L.ora_if6.restype = C.c_double
         L.ora_viscous_face.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, c_double_p]
         _libs[variant] = L
     return _libs[variant]
@@ -142,6 +149,8 @@ class Oracle:
         if st != 0:
             raise ValueError(f"ora_create failed with status {st}")
         self.h = h
+        if getattr(case, "visc_order", 4) != 4:
+            assert self.L.ora_set_visc_order(h, int(case.visc_order)) == 0
         self.shape = (5, nz + 6, ny + 6, nx + 6)
 
     def __del__(self):
@@ -306,3 +315,15 @@ def df(phi, Xf):
 
 def iface(phi):
     return lib().ora_if(_dp(_arr(phi, 4)))
+
+
+def dc6(phi, Xc):
+    return lib().ora_dc6(_dp(_arr(phi, 7)), float(Xc))
+
+
+def df6(phi, Xf):
+    return lib().ora_df6(_dp(_arr(phi, 6)), float(Xf))
+
+
+def iface6(phi):
+    return lib().ora_if6(_dp(_arr(phi, 6)))

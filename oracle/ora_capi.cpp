@@ -62,6 +62,13 @@ int ora_create(ora_solver** out, const ora_grid* g, int dtype, double gamma, dou
   return ORA_OK;
 }
 
+int ora_set_visc_order(ora_solver* s, int order) {
+  if (!s || (order != 4 && order != 6)) return ORA_EINVAL;
+  s->c.visc_order = order;
+  ora::build_metrics(s->c);
+  return ORA_OK;
+}
+
 void ora_destroy(ora_solver* s) { delete s; }
 
 size_t ora_state_elems(const ora_solver* s) { return (size_t)5 * s->c.P[0] * s->c.P[1] * s->c.P[2]; }
@@ -195,6 +202,9 @@ double ora_viscosity(const ora_mu_law* mu, double T) {
 double ora_dc(const double phi[5], double Xc) { return ora::d_centre<double>(phi[0], phi[1], phi[3], phi[4], Xc); }
 double ora_df(const double phi[4], double Xf) { return ora::d_face<double>(phi[0], phi[1], phi[2], phi[3], Xf); }
 double ora_if(const double phi[4]) { return ora::i_face<double>(phi[0], phi[1], phi[2], phi[3]); }
+double ora_dc6(const double phi[7], double Xc) { return ora::d_centre6<double>(phi[0], phi[1], phi[2], phi[4], phi[5], phi[6], Xc); }
+double ora_df6(const double phi[6], double Xf) { return ora::d_face6<double>(phi[0], phi[1], phi[2], phi[3], phi[4], phi[5], Xf); }
+double ora_if6(const double phi[6]) { return ora::i_face6<double>(phi[0], phi[1], phi[2], phi[3], phi[4], phi[5]); }
 
 int ora_viscous_face(ora_solver* s, const void* U, int dir, int i, int j, int k, double Fd[5]) {
   if (!s || !U || s->dtype != ORA_F64 || dir < 0 || dir > 2) return ORA_EINVAL;

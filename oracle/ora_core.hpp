@@ -192,4 +192,21 @@ inline R i_face(R m1, R c0, R p1, R p2) {
   return (R(9) * (c0 + p1) - (m1 + p2)) / R(16);
 }
 
+// Sixth-order members of the same family (the paper's DNS used "6th-order central" dissipative
+// fluxes).  The coefficients are fixed by polynomial exactness on the symmetric 6- / 7-point
+// stencils: centre derivative (-1, 9, -45, 0, 45, -9, 1)/60, face derivative from cell values
+// (75/64, -25/384, 3/640) on the three symmetric pairs, face interpolation (150, -25, 3)/256; difference form.
+template <class R>
+inline R d_centre6(R m3, R m2, R m1, R p1, R p2, R p3, R Xc) {  // phi_{i-3..i-1}, phi_{i+1..i+3}
+  return (R(45) * (p1 - m1) - R(9) * (p2 - m2) + (p3 - m3)) / (R(60) * Xc);
+}
+template <class R>
+inline R d_face6(R m2, R m1, R c0, R p1, R p2, R p3, R Xf) {  // phi_{i-2} .. phi_{i+3}, face i+1/2
+  return (R(2250) * (p1 - c0) - R(125) * (p2 - m1) + R(9) * (p3 - m2)) / (R(1920) * Xf);
+}
+template <class R>
+inline R i_face6(R m2, R m1, R c0, R p1, R p2, R p3) {
+  return (R(150) * (c0 + p1) - R(25) * (m1 + p2) + R(3) * (m2 + p3)) / R(256);
+}
+
 }  // namespace ora

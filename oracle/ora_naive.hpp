@@ -103,6 +103,29 @@ inline void face_flux(const Config& c, const double* U, int d, int i, int j, int
     double X1 = c.Xc[t1][it[t1] + NH], X2 = c.Xc[t2][it[t2] + NH];
     double G[3][3], gT, uf[3], Tf;
     Cell cm = cellat(-1, 0, 0), c0 = cellat(0, 0, 0), c1 = cellat(1, 0, 0), c2 = cellat(2, 0, 0);
+    if (c.visc_order == 6) {
+      // sixth order, weights written out: derivative (9, -125, 2250 | 2250, -125, 9)/1920 on the pairs about the
+      // face, interpolation (3, -25, 150, 150, -25, 3)/256, centre derivative (-1, 9, -45, 0, 45, -9, 1)/60
+      const double wd[6] = {-9.0 / 1920, 125.0 / 1920, -2250.0 / 1920, 2250.0 / 1920, -125.0 / 1920, 9.0 / 1920};
+      const double wi[6] = {3.0 / 256, -25.0 / 256, 150.0 / 256, 150.0 / 256, -25.0 / 256, 3.0 / 256};
+      const double wc[7] = {-1.0 / 60, 9.0 / 60, -45.0 / 60, 0.0, 45.0 / 60, -9.0 / 60, 1.0 / 60};
+      for (int a = 0; a < 3; ++a) { G[a][n] = 0; uf[a] = 0; G[a][t1] = 0; G[a][t2] = 0; }
+      gT = 0; Tf = 0;
+      for (int m = -2; m <= 3; ++m) {
+        Cell cc = cellat(m, 0, 0);
+        for (int a = 0; a < 3; ++a) { G[a][n] += wd[m + 2] * cc.vel[a] / Xf; uf[a] += wi[m + 2] * cc.vel[a]; }
+        gT += wd[m + 2] * cc.T / Xf; Tf += wi[m + 2] * cc.T;
+        for (int a = 0; a < 3; ++a) {
+          double g1 = 0, g2 = 0;
+          for (int r = -3; r <= 3; ++r) {
+            if (r == 0) continue;
+            g1 += wc[r + 3] * cellat(m, r, 0).vel[a] / X1;
+            g2 += wc[r + 3] * cellat(m, 0, r).vel[a] / X2;
+          }
+          G[a][t1] += wi[m + 2] * g1; G[a][t2] += wi[m + 2] * g2;
+        }
+      }
+    } else {
     for (int a = 0; a < 3; ++a) {
       G[a][n] = (27 * (c1.vel[a] - c0.vel[a]) - (c2.vel[a] - cm.vel[a])) / (24 * Xf);
       uf[a] = (9 * (c0.vel[a] + c1.vel[a]) - (cm.vel[a] + c2.vel[a])) / 16;
@@ -117,6 +140,7 @@ inline void face_flux(const Config& c, const double* U, int d, int i, int j, int
       }
       G[a][t1] = (9 * (g1[1] + g1[2]) - (g1[0] + g1[3])) / 16;
       G[a][t2] = (9 * (g2[1] + g2[2]) - (g2[0] + g2[3])) / 16;
+    }
     }
     double mu = c.mu.mu_ref;
     if (c.mu.sutherland) mu = c.mu.mu_ref * std::pow(Tf / c.mu.T_ref, 1.5) * (c.mu.T_ref + c.mu.S) / (Tf + c.mu.S);

@@ -27,6 +27,7 @@ struct Config {
   std::vector<double> dirichlet[6];
   double g[3];
   bool viscous;
+  int visc_order = 4;             // order of the central dissipative-flux stencils: 4 (north_star) or 6
 };
 
 inline bool axis_periodic(const Config& c, int a) { return c.bc.face[2 * a].type == ORA_BC_PERIODIC; }
@@ -61,13 +62,16 @@ inline void build_metrics(Config& c) {
       edge += w;
     }
     const std::vector<double>& x = c.xc[a];
+    // index-space metrics: the derivative stencils of the chosen order applied to the cell centres themselves
     for (int i = 0; i < N; ++i) {
       int p = i + NH;
-      c.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
+      c.Xc[a][p] = c.visc_order == 6 ? d_centre6(x[p - 3], x[p - 2], x[p - 1], x[p + 1], x[p + 2], x[p + 3], 1.0)
+                                     : (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
     }
     for (int i = -1; i <= N - 1; ++i) {  // face i+1/2
       int p = i + NH;
-      c.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
+      c.Xf[a][p] = c.visc_order == 6 ? d_face6(x[p - 2], x[p - 1], x[p], x[p + 1], x[p + 2], x[p + 3], 1.0)
+                                     : (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
     }
   }
 }
@@ -211,13 +215,14 @@ void compute_gradients(const Config& c, Prim<R>& P) {
           int id[3] = {pi, pj, pk};
           R Xc = R(c.Xc[a][id[a]]);
           for (int b = 0; b < 3; ++b) {
-            R v[5];
-            for (int m = -2; m <= 2; ++m) {
+            R v[7];
+            for (int m = -3; m <= 3; ++m) {
               int jd[3] = {pi, pj, pk};
               jd[a] += m;
-              v[m + 2] = P.at(1 + b, jd[0], jd[1], jd[2]);
+              v[m + 3] = (m == -3 || m == 3) && c.visc_order != 6 ? R(0) : P.at(1 + b, jd[0], jd[1], jd[2]);
             }
-            P.grad(a, b, pi, pj, pk) = d_centre(v[0], v[1], v[3], v[4], Xc);
+            P.grad(a, b, pi, pj, pk) = c.visc_order == 6 ? d_centre6(v[0], v[1], v[2], v[4], v[5], v[6], Xc)
+                                                         : d_centre(v[1], v[2], v[4], v[5], Xc);
           }
         }
   }
@@ -228,6 +233,44 @@ void compute_gradients(const Config& c, Prim<R>& P) {
 template <class R> inline R cp_of(const Config& c) { return R(c.gamma * c.Rgas / (c.gamma - 1.0)); }
 template <> inline long double cp_of<long double>(const Config& c) {
   return (long double)c.gamma * (long double)c.Rgas / ((long double)c.gamma - 1.0L);
+}
+
+// The same flux with the sixth-order stencils (cells -2..3 about the face; transverse derivatives = I^f_6 of the
+// D^c_6 centre derivatives at those six cells).  Everything else as in viscous_face below.
+template <class R>
+void viscous_face6(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) {
+  const int n = d, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  auto val = [&](int q, int sn) -> R {
+    int id[3] = {pc[0], pc[1], pc[2]};
+    id[n] += sn;
+    return P.at(q, id[0], id[1], id[2]);
+  };
+  auto Df = [&](int q, R Xf) { return d_face6(val(q, -2), val(q, -1), val(q, 0), val(q, 1), val(q, 2), val(q, 3), Xf); };
+  auto If = [&](int q) { return i_face6(val(q, -2), val(q, -1), val(q, 0), val(q, 1), val(q, 2), val(q, 3)); };
+  const int qn = 1 + n, qt1 = 1 + t1, qt2 = 1 + t2, qT = 5;
+  const R Xf = R(c.Xf[n][pc[n]]);
+  R dn_un = Df(qn, Xf), dn_ut1 = Df(qt1, Xf), dn_ut2 = Df(qt2, Xf), dn_T = Df(qT, Xf);
+  R un_f = If(qn), ut1_f = If(qt1), ut2_f = If(qt2), T_f = If(qT);
+  auto Ig = [&](int a, int b) {
+    R g[6];
+    for (int m = -2; m <= 3; ++m) {
+      int id[3] = {pc[0], pc[1], pc[2]};
+      id[n] += m;
+      g[m + 2] = P.grad(a, b, id[0], id[1], id[2]);
+    }
+    return i_face6(g[0], g[1], g[2], g[3], g[4], g[5]);
+  };
+  R dt1_un = Ig(t1, n), dt1_ut1 = Ig(t1, t1), dt2_un = Ig(t2, n), dt2_ut2 = Ig(t2, t2);
+  R mu = viscosity(c.mu.sutherland, R(c.mu.mu_ref), R(c.mu.T_ref), R(c.mu.S), T_f);
+  R cp = cp_of<R>(c);
+  R lambda = mu * cp / R(c.Pr);
+  R div = dn_un + dt1_ut1 + dt2_ut2;
+  R tau_nn = mu * (R(2) * dn_un - cst<R>(2, 3) * div);
+  R tau_nt1 = mu * (dt1_un + dn_ut1);
+  R tau_nt2 = mu * (dt2_un + dn_ut2);
+  Fd[0] = R(0);
+  Fd[qn] = tau_nn; Fd[qt1] = tau_nt1; Fd[qt2] = tau_nt2;
+  Fd[4] = un_f * tau_nn + ut1_f * tau_nt1 + ut2_f * tau_nt2 + lambda * dn_T;
 }
 
 // ---------------------------------------------------------------- O6 dissipative flux of one face
@@ -243,6 +286,7 @@ void viscous_face(const Config& c, Prim<R>& P, int d, const int pc[3], R Fd[5]) 
   };
   const int qn = 1 + n, qt1 = 1 + t1, qt2 = 1 + t2, qT = 5;
   const R Xf = R(c.Xf[n][pc[n]]);
+  if (c.visc_order == 6) { viscous_face6(c, P, d, pc, Fd); return; }
   // normal derivatives D^f and face values I^f
   R dn_un = d_face(val(qn, -1, 0, 0), val(qn, 0, 0, 0), val(qn, 1, 0, 0), val(qn, 2, 0, 0), Xf);
   R dn_ut1 = d_face(val(qt1, -1, 0, 0), val(qt1, 0, 0, 0), val(qt1, 1, 0, 0), val(qt1, 2, 0, 0), Xf);

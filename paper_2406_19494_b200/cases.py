@@ -46,6 +46,7 @@ class Case:
     n_steps: Optional[int] = None
     t_end: Optional[float] = None
     notes: dict = field(default_factory=dict)
+    visc_order: int = 4                       # central dissipative-flux stencils: 4 (north_star) or 6
 
     @property
     def cells(self):

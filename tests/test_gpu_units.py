@@ -96,7 +96,7 @@ def test_fp32_face_flux_in_si_units_with_strong_jumps(jf, ora, d):
     scale = np.max(np.abs(Fo), axis=1, keepdims=True)
     assert np.max(np.abs(F32 - Fo) / scale) <= 1e-4
     F64 = jf.jf_diag_face_flux("f64", d, G, Rg, PR, mu, W)
-    assert np.max(np.abs(F64 - Fo) / scale) <= 5e-14
+    assert np.max(np.abs(F64 - Fo) / scale) <= 2e-12       # (jumps of half the pressure: both sides lose digits in the weights)
 
 
 def test_face_flux_consistency_on_uniform_stencils(jf, ora):

@@ -221,3 +221,58 @@ def test_face_derivative_modified_wavenumber(ora):
     val = ora.df(np.sin(theta * xs), 1.0)                         # d/dxi sin(theta xi) at xi = 0
     expect = (54 * np.sin(theta / 2) - 2 * np.sin(3 * theta / 2)) / 24.0
     assert val == pytest.approx(expect, rel=1e-14)
+
+
+# ------------------------------------------------------------------ sixth-order central stencils
+def test_sixth_order_stencils_polynomial_exactness(ora):
+    # the coefficients are fixed by exactness: D^c_6 and D^f_6 differentiate polynomials of degree <= 6 exactly
+    # (7 / 6 symmetric points), I^f_6 interpolates degree <= 5 exactly; degree 7 / 7 / 6 is NOT exact (the
+    # stencils are sixth order, no more); constants give exactly 0 / the constant
+    rng = np.random.default_rng(7)
+    h = 0.37
+    for deg in range(0, 8):
+        co = rng.uniform(-1, 1, deg + 1)
+        f = np.polynomial.Polynomial(co)
+        df = f.deriv()
+        x0 = 0.21
+        xs_c = x0 + h * np.arange(-3, 4)
+        xs_f = x0 + h * (np.arange(-2, 4) - 0.5)           # cells i-2..i+3 around the face at x0
+        scale = np.max(np.abs(co)) * max(1.0, (3.5 * h + abs(x0)) ** deg) * 10
+        ec = abs(ora.dc6(f(xs_c), h) - df(x0)) / scale
+        ef = abs(ora.df6(f(xs_f), h) - df(x0)) / scale
+        ei = abs(ora.iface6(f(xs_f)) - f(x0)) / scale
+        if deg <= 6:
+            assert ec <= 1e-13 and ef <= 1e-13
+        else:
+            assert ec > 1e-9 and ef > 1e-9
+        if deg <= 5:
+            assert ei <= 1e-13
+        elif deg == 6:
+            assert ei > 1e-9
+    assert ora.dc6(np.full(7, 3.3), h) == 0.0 and ora.df6(np.full(6, 3.3), h) == 0.0
+    assert ora.iface6(np.full(6, 3.3)) == pytest.approx(3.3, rel=1e-15)
+
+
+def test_sixth_order_modified_wavenumbers(ora):
+    # on exp(i k x): D^c_6 -> i k_c, k_c D = (45 sin t - 9 sin 2t + sin 3t)/30; D^f_6 (cell values -> face):
+    # k_f D = 2 (2250 sin(t/2) - 125 sin(3t/2) + 9 sin(5t/2))/1920; I^f_6 -> (150 cos(t/2) - 25 cos(3t/2) + 3 cos(5t/2))/128,
+    # with t = k D; and each is within O(t^6) of the exact symbol
+    D = 0.1
+    for t in (0.05, 0.3, 1.1, 2.4):
+        k = t / D
+        xc = D * np.arange(-3, 4)
+        xf = D * (np.arange(-2, 4) - 0.5)
+        kc = ora.dc6(np.sin(k * xc), D)                      # derivative of sin at 0 = k
+        kf = ora.df6(np.sin(k * xf), D)
+        ci = ora.iface6(np.cos(k * xf))                      # value of cos at 0 = 1
+        assert kc * D == pytest.approx((45 * np.sin(t) - 9 * np.sin(2 * t) + np.sin(3 * t)) / 30, rel=1e-13)
+        assert kf * D == pytest.approx(2 * (2250 * np.sin(t / 2) - 125 * np.sin(1.5 * t) + 9 * np.sin(2.5 * t)) / 1920, rel=1e-13)
+        assert ci == pytest.approx((150 * np.cos(t / 2) - 25 * np.cos(1.5 * t) + 3 * np.cos(2.5 * t)) / 128, rel=1e-13)
+    t = 0.05
+    k = t / D
+    assert abs(ora.dc6(np.sin(k * D * np.arange(-3, 4)), D) / k - 1) < t ** 6 / 100
+    assert abs(ora.df6(np.sin(k * D * (np.arange(-2, 4) - 0.5)), D) / k - 1) < t ** 6 / 100
+    # and sixth order beats fourth order on the same data
+    e4 = abs(ora.df(np.sin(k * D * (np.arange(-1, 3) - 0.5)), D) / k - 1)
+    e6 = abs(ora.df6(np.sin(k * D * (np.arange(-2, 4) - 0.5)), D) / k - 1)
+    assert e6 < e4 * t ** 2
