@@ -136,6 +136,16 @@ jf_status jf_rk3_step(jf_solver *s, void *U_dev, double dt);
  * interior cell is non-finite or has rho <= 0 or p <= 0. */
 jf_status jf_cfl_dt(jf_solver *s, const void *U_dev, double cfl, double *dt_host);
 
+/* Order of the central stencils of the dissipative flux (a5): 4 (default; north_star) or 6 — the "6th-order central"
+ * dissipative fluxes the paper's DNS used.  The coefficients are fixed by
+ * polynomial exactness on the symmetric stencils: D^c_6 = (-1,9,-45,0,45,-9,1)/60, D^f_6 = (75/64, -25/384, 3/640)
+ * on the three cell pairs about the face, I^f_6 = (150,-25,3)/256; difference form, transverse derivatives = I^f_6
+ * of D^c_6, index-space metrics rebuilt with the same stencils.  A face then reads cells -3..2 about it: the same
+ * three halo layers as WENO5 (N_h of PAPER.md:80 stays 3).  Synchronises; rewrites the metric tables.  JF_EINVAL for
+ * other orders and for JF_F64_TANGENT with order 6.  (The paper's TENO6-A reconstruction is NOT provided: its
+ * constants are not in PAPER.md.) */
+jf_status jf_set_visc_order(jf_solver *s, int order);
+
 /* Device-resident time step: the same reduction, finished on the device (the last block forms dt), with NO host
  * synchronisation:   dt = min(jf_cfl_dt's value, t_end - t)   (t_end = NaN: no clipping),
  * stored in the solver's workspace together with the running time t <- t + dt (t starts at 0; jf_dev_time sets it).

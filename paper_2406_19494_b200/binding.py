@@ -46,7 +46,7 @@ class jf_bc(C.Structure):
 
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
-           "jf_rk3_step", "jf_cfl_dt", "jf_cfl_dt_dev", "jf_rk3_step_dev", "jf_dev_time", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
+           "jf_rk3_step", "jf_cfl_dt", "jf_cfl_dt_dev", "jf_rk3_step_dev", "jf_dev_time", "jf_set_visc_order", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
            "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_diag_metrics", "jf_version"]
 
@@ -108,6 +108,8 @@ def lib():
         L.jf_rk3_step_dev.argtypes = [C.c_void_p, C.c_void_p]
         L.jf_dev_time.restype = C.c_int
         L.jf_dev_time.argtypes = [C.c_void_p, C.c_int, c_double_p, c_double_p]
+        L.jf_set_visc_order.restype = C.c_int
+        L.jf_set_visc_order.argtypes = [C.c_void_p, C.c_int]
         L.jf_last_error.restype = C.c_char_p
         L.jf_last_error.argtypes = [C.c_void_p]
         L.jf_launch_count.restype = C.c_ulonglong
@@ -230,6 +232,8 @@ class Solver:
         if st != JF_OK:
             raise JFError(st, "jf_create")
         self.h = h
+        if getattr(case, "visc_order", 4) != 4:
+            self._check(L.jf_set_visc_order(h, int(case.visc_order)))
         nx, ny, nz = case.n
         self.shape = (5, nz + 6, ny + 6, nx + 6)
         assert L.jf_state_elems(h) == int(np.prod(self.shape))
@@ -295,6 +299,9 @@ class Solver:
         out = self.torch.empty((14, self.case.n[axis]), dtype=self.torch.float64, device=self.device)
         self._check(lib().jf_plane_sums(self.h, self._ptr(U), int(axis), C.c_void_p(out.data_ptr())))
         return out
+
+    def jf_set_visc_order(self, order):
+        self._check(lib().jf_set_visc_order(self.h, int(order)))
 
     def jf_set_tangent_seed(self, dA, dkappa):
         self._check(lib().jf_set_tangent_seed(self.h, float(dA), float(dkappa)))

@@ -30,7 +30,7 @@ struct Metrics {
 // face (nearest first) - the halo cells then have the geometry they have on the undivided grid; else null.
 // nbf[f]: for an exchange face across an interior cut, the neighbour's three face coordinates beyond the face.
 void build_metrics(const int n[3], const double* const xf[3], const bool periodic[3], const double* const nbw[6],
-                   const double* const nbf[6], Metrics& M) {
+                   const double* const nbf[6], int order, Metrics& M) {
   for (int a = 0; a < 3; ++a) {
     const int N = n[a], P = N + 2 * NH;
     std::vector<double>&d = M.dl[a], &x = M.xc[a];
@@ -52,8 +52,16 @@ void build_metrics(const int n[3], const double* const xf[3], const bool periodi
       double g0 = xf[a][N];
       for (int m = 1; m <= NH; ++m) { const double g1 = nbf[2 * a + 1][m - 1]; d[NH + N - 1 + m] = g1 - g0; x[NH + N - 1 + m] = 0.5 * (g0 + g1); g0 = g1; }
     }
-    for (int p = NH; p < NH + N; ++p) M.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
-    for (int p = NH - 1; p < NH + N; ++p) M.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
+    // index-space metrics: the derivative stencils of the dissipative flux (fourth or sixth order) applied to the centres
+    if (order == 6) {
+      for (int p = NH; p < NH + N; ++p)
+        M.Xc[a][p] = (45.0 * (x[p + 1] - x[p - 1]) - 9.0 * (x[p + 2] - x[p - 2]) + (x[p + 3] - x[p - 3])) / 60.0;
+      for (int p = NH - 1; p < NH + N; ++p)
+        M.Xf[a][p] = (2250.0 * (x[p + 1] - x[p]) - 125.0 * (x[p + 2] - x[p - 1]) + 9.0 * (x[p + 3] - x[p - 2])) / 1920.0;
+    } else {
+      for (int p = NH; p < NH + N; ++p) M.Xc[a][p] = (x[p - 2] - 8.0 * x[p - 1] + 8.0 * x[p + 1] - x[p + 2]) / 12.0;
+      for (int p = NH - 1; p < NH + N; ++p) M.Xf[a][p] = (x[p - 1] - 27.0 * x[p] + 27.0 * x[p + 1] - x[p + 2]) / 24.0;
+    }
   }
 }
 
@@ -135,6 +143,12 @@ struct jf_solver {
   std::string err;
   unsigned long long launches;
   int seg_len[3];
+  // geometry inputs kept for jf_set_visc_order (the metric tables depend on the order of the derivative stencils)
+  int visc_order = 4;
+  int n[3];
+  std::vector<double> xfh[3];
+  jf_bc bc_host;
+  char* ws = nullptr;
   // TMA-staged gradient pass (jf_tma.cuh): tensor maps per state-array base address (U, stage buffers A, B, ...)
   bool grad_tma = false;
   std::unordered_map<const void*, CUtensorMap> maps;
@@ -235,11 +249,14 @@ jf_status diag_face_flux(int dir, double gamma, double R_gas, double Pr, const j
   return JF_OK;
 }
 
+// Geometry tables of the solver's grid for the current order of the dissipative stencils -> workspace
+// (1/Delta, Delta, 1/(12 X_xi^c) | 1/(60 X_xi^c), 1/(24 X_xi^f) | 1/(1920 X_xi^f), centres).  Synchronous copies.
 template <class T>
-jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double R_gas, double Pr,
-                const jf_mu_law* mu, const jf_bc* bc, const double* ga, char* ws) {
-  const int n[3] = {g->nx, g->ny, g->nz};
-  const double* xf[3] = {g->xf, g->yf, g->zf};
+jf_status upload_tables(jf_solver* s, Impl<T>& I) {
+  const int* n = s->n;
+  const double* xf[3] = {s->xfh[0].data(), s->xfh[1].data(), s->xfh[2].data()};
+  const jf_bc* bc = &s->bc_host;
+  char* ws = s->ws;
   bool per[3];
   for (int a = 0; a < 3; ++a) per[a] = bc->face[2 * a].type == JF_BC_PERIODIC;
   const double* nbw[6];
@@ -250,19 +267,17 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
     nbw[f] = ex && !nbf[f] ? bc->face[f].nb_width : nullptr;
   }
   Metrics M;
-  build_metrics(n, xf, per, nbw, nbf, M);
+  build_metrics(n, xf, per, nbw, nbf, s->visc_order, M);
   Layout L = make_layout(n, sizeof(T));
   jf::Params<T>& P = I.P;
-  for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
-  P.sy = P.P[0]; P.sz = (long long)P.P[0] * P.P[1]; P.vol = P.sz * P.P[2];
-  fill_gas<T>(P.gas, gamma, R_gas, Pr, mu, ga);
+  const double kc = s->visc_order == 6 ? 60.0 : 12.0, kf = s->visc_order == 6 ? 1920.0 : 24.0;
   for (int a = 0; a < 3; ++a) {
     const int Pn = n[a] + 6;
     std::vector<T> t[4];
     for (int k = 0; k < 4; ++k) t[k].resize(Pn);
     for (int p = 0; p < Pn; ++p) {
       t[0][p] = T(1.0 / M.dl[a][p]); t[1][p] = T(M.dl[a][p]);
-      t[2][p] = T(1.0 / (12.0 * M.Xc[a][p])); t[3][p] = T(1.0 / (24.0 * M.Xf[a][p]));
+      t[2][p] = T(1.0 / (kc * M.Xc[a][p])); t[3][p] = T(1.0 / (kf * M.Xf[a][p]));
     }
     for (int k = 0; k < 4; ++k)
       JF_CUDA(s, cudaMemcpy(ws + L.tab_T[a][k], t[k].data(), Pn * sizeof(T), cudaMemcpyHostToDevice));
@@ -270,6 +285,26 @@ jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double
     P.inv_dl[a] = (const T*)(ws + L.tab_T[a][0]); P.dl[a] = (const T*)(ws + L.tab_T[a][1]);
     P.i12Xc[a] = (const T*)(ws + L.tab_T[a][2]); P.i24Xf[a] = (const T*)(ws + L.tab_T[a][3]);
     P.xc[a] = (const double*)(ws + L.tab_xc[a]);
+  }
+  return JF_OK;
+}
+
+template <class T>
+jf_status setup(jf_solver* s, Impl<T>& I, const jf_grid* g, double gamma, double R_gas, double Pr,
+                const jf_mu_law* mu, const jf_bc* bc, const double* ga, char* ws) {
+  const int n[3] = {g->nx, g->ny, g->nz};
+  const double* xf[3] = {g->xf, g->yf, g->zf};
+  for (int a = 0; a < 3; ++a) { s->n[a] = n[a]; s->xfh[a].assign(xf[a], xf[a] + n[a] + 1); }
+  s->bc_host = *bc;
+  s->ws = ws;
+  Layout L = make_layout(n, sizeof(T));
+  jf::Params<T>& P = I.P;
+  for (int a = 0; a < 3; ++a) { P.n[a] = n[a]; P.P[a] = n[a] + 6; }
+  P.sy = P.P[0]; P.sz = (long long)P.P[0] * P.P[1]; P.vol = P.sz * P.P[2];
+  fill_gas<T>(P.gas, gamma, R_gas, Pr, mu, ga);
+  {
+    const jf_status st = upload_tables<T>(s, I);
+    if (st != JF_OK) return st;
   }
   for (int f = 0; f < 6; ++f) {
     const jf_bc_face& b = bc->face[f];
@@ -457,7 +492,7 @@ template <>
 bool launch_grad_tma<float>(jf_solver*, Impl<float>&, const float*, dim3, int) { return false; }
 
 // R_NSE of Eq. 6.  rk == nullptr: R <- R_NSE(U).  Otherwise the z sweep applies the RK stage.
-template <class T, bool VISC>
+template <class T, bool VISC, int ORD = 4>
 jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
   const jf::Params<T>& P = I.P;
   const T* G = VISC ? I.G : nullptr;
@@ -470,31 +505,35 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
     if (nseg < 1) nseg = 1;
     const int Lz = (P.P[2] + nseg - 1) / nseg;
     dim3 grid((P.P[0] + jf::GM_TX - 1) / jf::GM_TX, (P.P[1] + jf::GM_TY - 1) / jf::GM_TY, (P.P[2] + Lz - 1) / Lz);
-    if (!(s->grad_tma && launch_grad_tma<T>(s, I, U, grid, Lz)))
-      jf::gradient_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
+    if constexpr (ORD == 6) {
+      jf::gradient6_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
+    } else {
+      if (!(s->grad_tma && launch_grad_tma<T>(s, I, U, grid, Lz)))
+        jf::gradient_kernel<T><<<grid, dim3(jf::GM_TX, jf::GM_TY), 0, s->stream>>>(P, U, I.G, Lz);
+    }
     s->launches += 1;
   }
   {
     Timed t(s, K_SWEEP_X);
     const int groups = (P.n[1] * P.n[2] + jf::XS_LINES - 1) / jf::XS_LINES;   // one warp per group of lines
     const size_t sh = (size_t)jf::XS_WARPS * (jf::XS<VISC>::NV * jf::XS_RING + jf::XS_CARRY) * sizeof(T);
-    jf::sweep_x_kernel<T, VISC><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
+    jf::sweep_x_kernel<T, VISC, ORD><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
-  const size_t sh = jf::yz_smem_bytes<T, VISC>();
+  const size_t sh = jf::yz_smem_bytes<T, VISC, ORD>();
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
   jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0), nullptr};
   {
     Timed t(s, K_SWEEP_Y);
     const int L = s->seg_len[1];
     dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, (P.n[2] + jf::YZ_TY - 1) / jf::YZ_TY, (P.n[1] + L - 1) / L);
-    jf::sweep_yz_kernel<T, 1, VISC, 0><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
+    jf::sweep_yz_kernel<T, 1, VISC, 0, ORD><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
   }
   {
     Timed t(s, K_SWEEP_Z);
     const int L = s->seg_len[2];
     dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, (P.n[1] + jf::YZ_TY - 1) / jf::YZ_TY, (P.n[2] + L - 1) / L);
-    if (rk) jf::sweep_yz_kernel<T, 2, VISC, 2><<<grid, blk, sh, s->stream>>>(P, U, G, R, *rk, L);
-    else jf::sweep_yz_kernel<T, 2, VISC, 1><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
+    if (rk) jf::sweep_yz_kernel<T, 2, VISC, 2, ORD><<<grid, blk, sh, s->stream>>>(P, U, G, R, *rk, L);
+    else jf::sweep_yz_kernel<T, 2, VISC, 1, ORD><<<grid, blk, sh, s->stream>>>(P, U, G, R, none, L);
   }
   s->launches += 3;
   JF_CUDA(s, cudaPeekAtLastError());
@@ -503,9 +542,9 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
 
 // The viscous y/z sweeps keep a 5-cell window of 10 values per thread in shared memory (50 KB per
 // 128-thread block in fp64): above the 48 KB default, so opt in once per solver.
-template <class T, bool VISC>
+template <class T, bool VISC, int ORD = 4>
 cudaError_t opt_in_smem() {
-  const int sh = (int)jf::yz_smem_bytes<T, VISC>();
+  const int sh = (int)jf::yz_smem_bytes<T, VISC, ORD>();
   cudaError_t e = cudaSuccess;
   auto set = [&](const void* f) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
@@ -515,14 +554,25 @@ cudaError_t opt_in_smem() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, JF_YZ_CARVEOUT);
 #endif
   };
-  set((const void*)jf::sweep_yz_kernel<T, 1, VISC, 0>);
-  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 1>);
-  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 2>);
+  set((const void*)jf::sweep_yz_kernel<T, 1, VISC, 0, ORD>);
+  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 1, ORD>);
+  set((const void*)jf::sweep_yz_kernel<T, 2, VISC, 2, ORD>);
   return e;
+}
+
+// sixth-order dissipative flux: fp64 / fp32 only (jf_set_visc_order refuses the tangent type)
+template <class T>
+jf_status launch_rhs_o6(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
+  return launch_rhs_t<T, true, 6>(s, I, U, R, rk);
+}
+template <>
+jf_status launch_rhs_o6<jf::Dual>(jf_solver* s, Impl<jf::Dual>&, const jf::Dual*, jf::Dual*, const jf::RKArgs<jf::Dual>*) {
+  return fail(s, JF_EINVAL, "sixth-order dissipative flux: not built for the tangent type");
 }
 
 template <class T>
 jf_status launch_rhs(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKArgs<T>* rk) {
+  if (s->viscous && s->visc_order == 6) return launch_rhs_o6<T>(s, I, U, R, rk);
   return s->viscous ? launch_rhs_t<T, true>(s, I, U, R, rk) : launch_rhs_t<T, false>(s, I, U, R, rk);
 }
 
@@ -837,6 +887,24 @@ jf_status jf_rk3_step(jf_solver* s, void* U, double dt) {
   return s->dtype == JF_F64   ? rk3<double>(s, s->d, (double*)U, dt, false)
          : s->dtype == JF_F32 ? rk3<float>(s, s->f, (float*)U, dt, false)
                               : rk3<jf::Dual>(s, s->t, (jf::Dual*)U, dt, false);
+}
+
+jf_status jf_set_visc_order(jf_solver* s, int order) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  if (order != 4 && order != 6) return fail(s, JF_EINVAL, "jf_set_visc_order: order must be 4 or 6");
+  if (order == 6 && s->dtype == JF_F64_TANGENT) return fail(s, JF_EINVAL, "jf_set_visc_order: order 6 is not built for the tangent type");
+  if (order == s->visc_order) return JF_OK;
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  s->visc_order = order;
+  for (auto& g : s->graphs) cudaGraphExecDestroy(g.exec);      // the captured steps launch the other kernels
+  s->graphs.clear();
+  if (order == 6 && s->viscous) {
+    const cudaError_t ce = s->dtype == JF_F64 ? opt_in_smem<double, true, 6>() : opt_in_smem<float, true, 6>();
+    if (ce != cudaSuccess) return fail(s, JF_ECUDA, "cudaFuncSetAttribute", ce);
+  }
+  return s->dtype == JF_F64 ? upload_tables<double>(s, s->d) : s->dtype == JF_F32 ? upload_tables<float>(s, s->f)
+                                                                                  : upload_tables<jf::Dual>(s, s->t);
 }
 
 jf_status jf_cfl_dt_dev(jf_solver* s, const void* U, double cflnum, double t_end) {

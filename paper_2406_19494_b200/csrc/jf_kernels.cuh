@@ -19,6 +19,19 @@ namespace jf {
 
 constexpr int NH = 3;
 
+// Tangent type (value, tangent): twice the registers per value.  The marching sweeps hold 100 KB of window per block,
+// so two blocks per SM is all that fits in shared memory anyway: give them the 255 registers that leaves (at the
+// primal's 168 they spilled 450-650 bytes per thread); the x sweep likewise runs 2 blocks of 4 warps at 255.
+#ifndef JF_XS_MINB_DUAL
+#define JF_XS_MINB_DUAL 2
+#endif
+#ifndef JF_YZ_MINB_DUAL
+#define JF_YZ_MINB_DUAL 2
+#endif
+#ifndef JF_GM_MINB_DUAL
+#define JF_GM_MINB_DUAL 2
+#endif
+
 template <class T>
 struct Params {
   int n[3], P[3];
@@ -284,7 +297,7 @@ struct alignas(sizeof(T) >= 8 ? 16 : 2 * sizeof(T)) Pair2 { T a, b; };
 #endif
 constexpr int GM_TX = 32, GM_TY = JF_GM_TY, GM_SX = GM_TX + 4, GM_SY = GM_TY + 4, GM_RIM = GM_SX * GM_SY - GM_TX * GM_TY;
 template <class T>
-__global__ void __launch_bounds__(GM_TX * GM_TY, sizeof(T) > 8 ? 1 : JF_GM_MINB)
+__global__ void __launch_bounds__(GM_TX * GM_TY, sizeof(T) > 8 ? JF_GM_MINB_DUAL : JF_GM_MINB)
 gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz) {
   __shared__ T sv[2][3][GM_SY][GM_SX];
   // thread-private queue of (d_x u, d_y v) of planes p-2, p-1: shared memory (the registers are full at 3 blocks
@@ -390,6 +403,97 @@ gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz)
   }
 }
 
+// ------------------------------------------------------------------ a5 (part) centre gradients, sixth order
+// The same nine outputs with D^c_6 = [45 (+1 - -1) - 9 (+2 - -2) + (+3 - -3)]/(60 X_xi^c) (SURVEY 8(f)
+// rank 3; the table i12Xc then holds 1/(60 X_xi^c)).  Same plane march with a 3-cell rim and a seven-deep register
+// queue; written for clarity, not tuned (this is the "next" row, not the north_star path): every thread converts
+// up to three cells of the (GM_TX + 6) x (GM_TY + 6) plane, double-buffered, one __syncthreads per plane.
+constexpr int G6_SX = GM_TX + 6, G6_SY = GM_TY + 6;
+template <class T>
+__global__ void __launch_bounds__(GM_TX * GM_TY, sizeof(T) > 8 ? 1 : 2)
+gradient6_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz) {
+  __shared__ T sv[2][3][G6_SY][G6_SX];
+  T dq[3][2];                                  // (d_x u, d_y v) of planes p-3, p-2, p-1
+#pragma unroll
+  for (int a = 0; a < 3; ++a) dq[a][0] = dq[a][1] = T(0);
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * GM_TX + tx;
+  const int x0 = blockIdx.x * GM_TX, y0 = blockIdx.y * GM_TY;
+  const int px = x0 + tx, py = y0 + ty;
+  const int Px = P.P[0], Py = P.P[1], Pz = P.P[2];
+  const int k0 = blockIdx.z * Lz, k1 = min(k0 + Lz, Pz);
+  const bool own = px < Px && py < Py;
+  const unsigned o_own = (unsigned)py * (unsigned)P.sy + (unsigned)px;
+  const unsigned sz = (unsigned)P.sz;
+  const bool dx_ok = own && px >= NH && px < P.n[0] + NH, dy_ok = own && py >= NH && py < P.n[1] + NH;
+  const T scx = dx_ok ? P.i12Xc[0][px] : T(0), scy = dy_ok ? P.i12Xc[1][py] : T(0);
+  T q[7][3];                                   // (u,v,w) of the own cell at planes p-6 .. p
+#pragma unroll
+  for (int a = 0; a < 7; ++a) q[a][0] = q[a][1] = q[a][2] = T(0);
+  const int pstart = max(k0 - 3, 0), pend = min(k1 + 2, Pz - 1);
+  constexpr int NCELL = G6_SX * G6_SY, NTHR = GM_TX * GM_TY;
+  for (int p = pstart; p <= pend; ++p) {
+    const int b = p & 1;
+#pragma unroll
+    for (int r = 0; r < (NCELL + NTHR - 1) / NTHR; ++r) {
+      const int c = tid + r * NTHR;
+      if (c < NCELL) {
+        const int cy = c / G6_SX, cx = c - cy * G6_SX;
+        const int gx = x0 - 3 + cx, gy = y0 - 3 + cy;
+        const bool in = gx >= 0 && gx < Px && gy >= 0 && gy < Py;
+        const unsigned o = (unsigned)gy * (unsigned)P.sy + (unsigned)gx + (unsigned)p * sz;
+        const T ri = Num<T>::rcp(in ? U[o] : T(1));
+        sv[b][0][cy][cx] = in ? (U + P.vol)[o] * ri : T(0);
+        sv[b][1][cy][cx] = in ? (U + 2 * P.vol)[o] * ri : T(0);
+        sv[b][2][cy][cx] = in ? (U + 3 * P.vol)[o] * ri : T(0);
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int a = 0; a < 6; ++a) { q[a][0] = q[a + 1][0]; q[a][1] = q[a + 1][1]; q[a][2] = q[a + 1][2]; }
+    q[6][0] = sv[b][0][ty + 3][tx + 3]; q[6][1] = sv[b][1][ty + 3][tx + 3]; q[6][2] = sv[b][2][ty + 3][tx + 3];
+    const unsigned op = o_own + (unsigned)p * sz;
+    T dxu = T(0), dyv = T(0);
+    if (p >= k0 && p < k1) {
+      if (dx_ok) {
+        T d[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const T* r = &sv[b][c][ty + 3][tx + 3];
+          d[c] = (T(45) * (r[1] - r[-1]) - T(9) * (r[2] - r[-2]) + (r[3] - r[-3])) * scx;
+        }
+        dxu = d[0];
+        (G + (long long)1 * P.vol)[op] = d[1];
+        (G + (long long)2 * P.vol)[op] = d[2];
+      }
+      if (dy_ok) {
+        T d[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const T* r = &sv[b][c][ty + 3][tx + 3];
+          d[c] = (T(45) * (r[G6_SX] - r[-G6_SX]) - T(9) * (r[2 * G6_SX] - r[-2 * G6_SX]) + (r[3 * G6_SX] - r[-3 * G6_SX])) * scy;
+        }
+        dyv = d[1];
+        (G + (long long)3 * P.vol)[op] = d[0];
+        (G + (long long)5 * P.vol)[op] = d[2];
+      }
+      if (dx_ok && dy_ok) (G + (long long)8 * P.vol)[op] = dxu + dyv;
+    }
+    const int pzc = p - 3;                     // plane whose z derivative is complete now
+    if (own && pzc >= k0 && pzc < k1 && pzc >= NH && pzc < P.n[2] + NH && p - 6 >= pstart) {
+      const T scz = P.i12Xc[2][pzc];
+      T d[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) d[c] = (T(45) * (q[4][c] - q[2][c]) - T(9) * (q[5][c] - q[1][c]) + (q[6][c] - q[0][c])) * scz;
+      const unsigned oz = op - 3u * sz;
+      (G + (long long)6 * P.vol)[oz] = d[0];
+      (G + (long long)7 * P.vol)[oz] = d[1];
+      if (dy_ok) (G + (long long)0 * P.vol)[oz] = dq[0][1] + d[2];
+      if (dx_ok) (G + (long long)4 * P.vol)[oz] = d[2] + dq[0][0];
+    }
+    dq[0][0] = dq[1][0]; dq[0][1] = dq[1][1]; dq[1][0] = dq[2][0]; dq[1][1] = dq[2][1]; dq[2][0] = dxu; dq[2][1] = dyv;
+  }
+}
+
 template <class T>
 struct RKArgs {
   const T* Un;   // U^n
@@ -427,8 +531,8 @@ struct RKArgs {
 #endif
 constexpr int XS_WARPS = JF_XS_WARPS, XS_RING = 64, XS_LINES = JF_XS_LINES, XS_CARRY = 10;
 template <bool VISC> struct XS { static constexpr int NV = VISC ? 9 : 5; };
-template <class T, bool VISC>
-__global__ void __launch_bounds__(XS_WARPS * 32, sizeof(T) == 4 ? JF_XS_MINB_F32 : JF_XS_MINB)
+template <class T, bool VISC, int ORD = 4>
+__global__ void __launch_bounds__(XS_WARPS * 32, sizeof(T) == 4 ? JF_XS_MINB_F32 : sizeof(T) > 8 ? JF_XS_MINB_DUAL : JF_XS_MINB)
 sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* __restrict__ R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NV = XS<VISC>::NV;           // rho,u,v,w,p [,T, d_y u, d_z u, d_y v + d_z w]
@@ -519,9 +623,9 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
     T F[5] = {T(0), T(0), T(0), T(0), T(0)};
 #ifdef JF_XS_BRANCHY
     if (cell && pc >= 3)
-      face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][pc - 1] : T(0), F);
+      face_flux<T, 0, VISC, ORD>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][pc - 1] : T(0), F);
 #else
-    face_flux<T, 0, VISC>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][min(max(pc - 1, 0), Px - 1)] : T(0), F);
+    face_flux<T, 0, VISC, ORD>(gas, WL, Wp, w, g, VISC ? P.i24Xf[0][min(max(pc - 1, 0), Px - 1)] : T(0), F);
 #endif
     const bool upd = cell && pc >= 4;
     const T idl = upd ? P.inv_dl[0][pc - 1] : T(0);
@@ -564,21 +668,21 @@ sweep_x_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T*
 #ifndef JF_YZ_PAIR_MASK
 #define JF_YZ_PAIR_MASK 3
 #endif
-constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY, YZ_RING = 5;
+constexpr int YZ_TX = 32, YZ_TY = JF_YZ_TY;
+// window depth: cells c-2..c+2 (WENO5 of cell c; the fourth-order dissipative flux of face c-1/2 reads c-2..c+1);
+// the sixth-order dissipative flux reads c-3..c+2: one more slot
+__host__ __device__ constexpr int yz_ring(int ORD) { return ORD == 6 ? 6 : 5; }
 template <bool VISC> struct YZ { static constexpr int NP = VISC ? 5 : 3; };   // pairs per window cell
-template <class T, bool VISC>
+template <class T, bool VISC, int ORD = 4>
 constexpr size_t yz_smem_bytes() {
-  size_t b = (size_t)YZ_RING * YZ<VISC>::NP * YZ_TX * YZ_TY * sizeof(Pair2<T>);
-#ifdef JF_YZ_FSMEM
-  b += (size_t)5 * YZ_TX * YZ_TY * sizeof(T);
-#endif
-  return b;
+  return (size_t)yz_ring(ORD) * YZ<VISC>::NP * YZ_TX * YZ_TY * sizeof(Pair2<T>);
 }
-template <class T, int DIR, bool VISC, int MODE>
-__global__ void __launch_bounds__(YZ_TX * YZ_TY, sizeof(T) == 4 ? JF_YZ_MINB_F32 : JF_YZ_MINB)
+template <class T, int DIR, bool VISC, int MODE, int ORD = 4>
+__global__ void __launch_bounds__(YZ_TX * YZ_TY, sizeof(T) == 4 ? JF_YZ_MINB_F32 : sizeof(T) > 8 ? JF_YZ_MINB_DUAL : JF_YZ_MINB)
 sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T* R, RKArgs<T> rk, int L) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using P2 = Pair2<T>;
+  constexpr int YZ_RING = yz_ring(ORD), LO = YZ_RING - 3;   // slots hold cells c-LO .. c+2
   constexpr bool PAIR = (JF_YZ_PAIR_MASK >> MODE) & 1;   // window stored as pairs (128-bit accesses) or as scalars
   P2* ring = reinterpret_cast<P2*>(smem_raw);  // [5 slots][NP pairs][threads]  (scalar: [5 slots][2 NP][threads])
   constexpr int NT = YZ_TX * YZ_TY, NP = YZ<VISC>::NP;
@@ -624,12 +728,13 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     }
   };
   T raw[5], gn[3] = {T(0), T(0), T(0)};
-  // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots 0..4.
+  // window of the first cell c0-1 (padded c0+2): padded cells c0 .. c0+4 -> slots LO-2 .. LO+2 (ORD 6: slot 0, the
+  // cell c0-4, is not read before it is replaced: the first face, c0-1/2, is formed one step later).
   // All loads are issued before the first conversion so that their latencies overlap.
   {
-    T raws[YZ_RING][5], gns[YZ_RING][3];
+    T raws[5][5], gns[5][3];
 #pragma unroll
-    for (int s = 0; s < YZ_RING; ++s) {
+    for (int s = 0; s < 5; ++s) {
       const unsigned o = col + (unsigned)(c0 + s) * sm;
 #pragma unroll
       for (int q = 0; q < 5; ++q) raws[s][q] = (MODE == 2) ? (U + q * P.vol)[o] : ld_stream((U + q * P.vol) + o);
@@ -637,34 +742,31 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       for (int c = 0; c < 3; ++c) gns[s][c] = VISC ? ld_stream(gsrc[c] + o) : T(0);
     }
 #pragma unroll
-    for (int s = 0; s < YZ_RING; ++s) put(s, raws[s], gns[s]);
+    for (int s = 0; s < 5; ++s) put(s + LO - 2, raws[s], gns[s]);
   }
-  // W^-_{c+1/2} of the previous step and (JF_YZ_FSMEM) the previous face flux are handed from step to step through
-  // thread-private shared memory instead of registers: variable q lives in the unused tenth value of ring slot q
-  // (the flux in five more words after the ring).  20 (40) registers and the 10 (20) rotation moves per step go.
+  // W^-_{c+1/2} of the previous step is handed from step to step either in registers (fp64 / fp32) or, for the
+  // tangent type (four registers per value), through thread-private shared memory: variable q lives in the unused
+  // tenth value of ring slot q.  (For fp64 the exchange was measured, also with 4 blocks per SM at 128 registers,
+  // which it makes spill-free: y 1.91 -> 1.99 ms, z + RK 2.15 -> 2.21 ms per step at 256^3; not used there.)
 #ifdef JF_YZ_XCHG
+  constexpr bool XCHG = true;
+#else
+  constexpr bool XCHG = sizeof(T) > 8;
+#endif
   auto xw = [&](int q) -> T* {
     if (PAIR) return &(mine + q * (NP * NT) + (NP - 1) * NT)->b;
     return mine1 + q * (2 * NP * NT) + (2 * NP - 1) * NT;
   };
-  static_assert(!VISC || NP == 5, "pad slot");
-#pragma unroll
-  for (int q = 0; q < 5; ++q) *xw(q) = T(1);
-#else
   T WmPrev[5];
 #pragma unroll
-  for (int q = 0; q < 5; ++q) WmPrev[q] = T(1);
-#endif
-#ifdef JF_YZ_FSMEM
-  T* fsm = reinterpret_cast<T*>(smem_raw + (size_t)YZ_RING * NP * NT * sizeof(P2)) + tid;
-#pragma unroll
-  for (int q = 0; q < 5; ++q) fsm[q * NT] = T(0);
-#else
+  for (int q = 0; q < 5; ++q) {
+    WmPrev[q] = T(1);
+    if (XCHG) *xw(q) = T(1);
+  }
   T Fprev[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) Fprev[q] = T(0);
-#endif
-  int s0 = 0;                                // slot of cell c-2
+  int s0 = 0;                                // slot of cell c-LO
   // metric table entries of the face / cell the NEXT step treats, loaded one step ahead (a per-step
   // scalar load issued where it is used stalls the warp for an L2 round trip: 11-13 % of all stall samples)
   T xf_n = VISC ? P.i24Xf[DIR][c0 - 1 + NH - 1] : T(0), idl_n = P.inv_dl[DIR][c0 - 1 + NH - 1];
@@ -680,22 +782,21 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
       for (int m = 0; m < YZ_RING; ++m) { slot[m] = s * (NP * NT); s = (s == YZ_RING - 1) ? 0 : s + 1; }
     }
     auto w = [&](int m, int q) -> T {
-      if (!PAIR) return mine1[2 * slot[m + 2] + q * NT];
-      const P2 v = mine[slot[m + 2] + (q >> 1) * NT];
+      if (!PAIR) return mine1[2 * slot[m + LO] + q * NT];
+      const P2 v = mine[slot[m + LO] + (q >> 1) * NT];
       return (q & 1) ? v.b : v.a;
     };
     auto g = [&](int m, int cc) -> T {
-      if (!PAIR) return mine1[2 * slot[m + 2] + (6 + cc) * NT];
-      const P2 v = mine[slot[m + 2] + (3 + (cc >> 1)) * NT];
+      if (!PAIR) return mine1[2 * slot[m + LO] + (6 + cc) * NT];
+      const P2 v = mine[slot[m + LO] + (3 + (cc >> 1)) * NT];
       return (cc & 1) ? v.b : v.a;
     };
     T Wm[5], Wp[5];
     weno_cell_states<T, DIR>(w, Wm, Wp);
-#ifdef JF_YZ_XCHG
-    T WmPrev[5];
+    if (XCHG) {
 #pragma unroll
-    for (int q = 0; q < 5; ++q) { T* x = xw(q); WmPrev[q] = *x; *x = Wm[q]; }
-#endif
+      for (int q = 0; q < 5; ++q) { T* x = xw(q); WmPrev[q] = *x; *x = Wm[q]; }
+    }
     // issue the loads this step consumes at its end
     const bool more = c < c1;                // another cell follows: its window needs padded pc+3
     const bool upd = c > c0;                 // cell c-1 is in [c0, c1): update it
@@ -720,16 +821,12 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
     }
     if (c >= c0) {                           // face c-1/2
       T F[5];
-      face_flux<T, DIR, VISC>(gas, WmPrev, Wp, w, g, xf_c, F);
+      face_flux<T, DIR, VISC, ORD>(gas, WmPrev, Wp, w, g, xf_c, F);
       if (upd) {
         const T idl = idl_c;
         T Rv[5];
 #pragma unroll
-#ifdef JF_YZ_FSMEM
-        for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - fsm[q * NT]) * idl;
-#else
         for (int q = 0; q < 5; ++q) Rv[q] = Rold[q] - (F[q] - Fprev[q]) * idl;
-#endif
         if (MODE >= 1 && gas.has_g) {
           T rho = w(-1, 0), u = w(-1, 1), v = w(-1, 2), ww = w(-1, 3);
           Rv[1] += rho * gas.g[0]; Rv[2] += rho * gas.g[1]; Rv[3] += rho * gas.g[2];
@@ -749,17 +846,13 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
         }
       }
 #pragma unroll
-#ifdef JF_YZ_FSMEM
-      for (int q = 0; q < 5; ++q) fsm[q * NT] = F[q];
-#else
       for (int q = 0; q < 5; ++q) Fprev[q] = F[q];
-#endif
     }
-#ifndef JF_YZ_XCHG
+    if (!XCHG) {
 #pragma unroll
-    for (int q = 0; q < 5; ++q) WmPrev[q] = Wm[q];
-#endif
-    if (more) put(s0, raw, gn);              // cell c+3 replaces cell c-2
+      for (int q = 0; q < 5; ++q) WmPrev[q] = Wm[q];
+    }
+    if (more) put(s0, raw, gn);              // cell c+3 replaces cell c-LO
     s0 = (s0 == YZ_RING - 1) ? 0 : s0 + 1;
   }
 }

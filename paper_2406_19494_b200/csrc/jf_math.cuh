@@ -265,33 +265,47 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
 //            c = 0: d_t1 u_n, 1: d_t2 u_n, 2: d_t1 u_t1 + d_t2 u_t2 (tau_nn needs only the sum, and the
 //            face interpolation is linear, so the gradient pass stores the sum: 3 arrays per sweep, not 4)
 //   i24Xf: 1/(24 X_xi^f) of this face.   (n,t1,t2) = (DIR, DIR+1, DIR+2) mod 3.
-template <class T, int DIR, class WAcc, class GAcc>
+template <class T, int DIR, int ORD, class WAcc, class GAcc>
 __device__ __forceinline__ void viscous_sub(const Gas<T>& gas, const WAcc& w, const GAcc& g, T i24Xf, T Fr[5]) {
   constexpr int n = DIR, t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   // Unscaled stencil sums: dn = 24 X_xi^f * (normal derivative), fv = 16 * (face value), gt = 16 * (face
   // interpolation of the transverse centre derivative) of u_n, u_t1, u_t2, T; the scale factors are folded
   // into mX = mu/(24 X_xi^f) and mG = mu/16.
+  // ORD == 6: the sixth-order members on cells -3..2 about the face,
+  // dn = 1920 X_xi^f d_n = 2250 (0 - -1) - 125 (1 - -2) + 9 (2 - -3), fv = 256 I^f = 150 (-1 + 0) - 25 (-2 + 1) + 3 (-3 + 2);
+  // the table then holds 1/(1920 X_xi^f) and the interpolation scale is 1/256.
   T dn[4], fv[4];
   constexpr int qv[4] = {1 + n, 1 + t1, 1 + t2, 5};
+  constexpr double ISC = ORD == 6 ? 1.0 / 256.0 : 1.0 / 16.0;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     T m1 = w(-2, qv[c]), c0 = w(-1, qv[c]), p1 = w(0, qv[c]), p2 = w(1, qv[c]);
-    dn[c] = Num<T>::fma_(T(27), p1 - c0, m1 - p2);
-    fv[c] = Num<T>::fma_(T(9), c0 + p1, -(m1 + p2));
+    if (ORD == 6) {
+      T m2 = w(-3, qv[c]), p3 = w(2, qv[c]);
+      dn[c] = Num<T>::fma_(T(2250), p1 - c0, Num<T>::fma_(T(-125), p2 - m1, T(9) * (p3 - m2)));
+      fv[c] = Num<T>::fma_(T(150), c0 + p1, Num<T>::fma_(T(-25), m1 + p2, T(3) * (m2 + p3)));
+    } else {
+      dn[c] = Num<T>::fma_(T(27), p1 - c0, m1 - p2);
+      fv[c] = Num<T>::fma_(T(9), c0 + p1, -(m1 + p2));
+    }
   }
   T gt[3];
 #pragma unroll
-  for (int c = 0; c < 3; ++c)
-    gt[c] = Num<T>::fma_(T(9), g(-1, c) + g(0, c), -(g(-2, c) + g(1, c)));
-  T mu = gas.sutherland ? viscosity<T>(gas, fv[3] * T(1.0 / 16.0)) : gas.mu_ref;
-  T mX = mu * i24Xf, mG = mu * T(1.0 / 16.0);
+  for (int c = 0; c < 3; ++c) {
+    if (ORD == 6)
+      gt[c] = Num<T>::fma_(T(150), g(-1, c) + g(0, c), Num<T>::fma_(T(-25), g(-2, c) + g(1, c), T(3) * (g(-3, c) + g(2, c))));
+    else
+      gt[c] = Num<T>::fma_(T(9), g(-1, c) + g(0, c), -(g(-2, c) + g(1, c)));
+  }
+  T mu = gas.sutherland ? viscosity<T>(gas, fv[3] * T(ISC)) : gas.mu_ref;
+  T mX = mu * i24Xf, mG = mu * T(ISC);
   // tau_nn = mu (2 d_n u_n - 2/3 div) = mu (4/3 d_n u_n - 2/3 (d_t1 u_t1 + d_t2 u_t2))
   T tnn = Num<T>::fma_(mX * Num<T>::template K<K_4_3>(), dn[0], -(mG * Num<T>::template K<K_2_3>()) * gt[2]);
   T tn1 = Num<T>::fma_(mX, dn[1], mG * gt[0]);
   T tn2 = Num<T>::fma_(mX, dn[2], mG * gt[1]);
   Fr[1] -= tnn; Fr[2] -= tn1; Fr[3] -= tn2;
   T work = Num<T>::fma_(fv[2], tn2, Num<T>::fma_(fv[1], tn1, fv[0] * tnn));
-  Fr[4] = Num<T>::fma_(-(mX * gas.lam_fac), dn[3], Num<T>::fma_(T(-1.0 / 16.0), work, Fr[4]));
+  Fr[4] = Num<T>::fma_(-(mX * gas.lam_fac), dn[3], Num<T>::fma_(T(-ISC), work, Fr[4]));
 }
 
 // Rotated-frame component order of direction DIR: slot c of (rho, u_n, u_t1, u_t2, p) is
@@ -314,12 +328,12 @@ __device__ __forceinline__ void weno_cell_states(const WAcc& w, T Wm[5], T Wp[5]
 
 // Total face flux F = F^c - F^d (Eq. 6) of the face between cells -1 | 0 from its rotated
 // left / right states; un-rotated into (rho, rho u, rho v, rho w, E) slots.
-template <class T, int DIR, bool VISC, class WAcc, class GAcc>
+template <class T, int DIR, bool VISC, int ORD = 4, class WAcc, class GAcc>
 __device__ __forceinline__ void face_flux(const Gas<T>& gas, const T WL[5], const T WR[5], const WAcc& w,
                                           const GAcc& g, T i24Xf, T F[5]) {
   T Fr[5];
   hllc_rot<T>(gas, WL, WR, Fr);
-  if (VISC) viscous_sub<T, DIR>(gas, w, g, i24Xf, Fr);
+  if (VISC) viscous_sub<T, DIR, ORD>(gas, w, g, i24Xf, Fr);
 #pragma unroll
   for (int c = 0; c < 5; ++c) F[rot_q<DIR>(c)] = Fr[c];
 }
