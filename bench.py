@@ -42,6 +42,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sweep", dest="sweep", action="store_false",
                     help="skip the other lines of configs[4] (384^3, 512^3 fp64, 512^3 fp32) the default run appends")
+    ap.add_argument("--visc-order", type=int, default=4, choices=[4, 6],
+                    help="order of the central dissipative-flux stencils: 4 (north_star, default) or 6 (PAPER.md:90, the "
+                         "paper's DNS; with --case channel --dtype f32 this is the paper's own precision and dissipative scheme)")
     ap.add_argument("--decomp", default=None, metavar="Sx,Sy,Sz",
                     help="block-decomposition arm: one --size^3 block per rank, Sx*Sy*Sz ranks (PAPER.md:78-82)")
     return ap.parse_args()
@@ -109,11 +112,12 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------- reference arm = the oracle
-def oracle_throughput(n, steps, warmup, channel=False):
+def oracle_throughput(n, steps, warmup, channel=False, visc_order=4):
     """The oracle as it stands (oracle/libora.so, -O2 -ffp-contract=off -fopenmp) on the host cores."""
     from oracle import ora
     from paper_2406_19494_b200 import cases
     case = cases.channel() if channel else cases.tgv(n)
+    case.visc_order = visc_order
     o = ora.Oracle(case)
     U = o.state()
 
@@ -246,6 +250,7 @@ def run_ours(args):
     n, K, W = args.size, args.steps, max(args.warmup, 3)
     channel = args.case == "channel"
     case = cases.channel() if channel else cases.tgv(n)
+    case.visc_order = args.visc_order
     solver = jf.Solver(case, args.dtype, device=str(dev))
     esz = 8 if args.dtype == "f64" else 4
     U = solver.state()
@@ -362,7 +367,7 @@ def run_ours(args):
     fm = flop_model(n)
     if channel:                                        # one step of config 2, counted by the oracle at full size
         with open(os.path.join(ROOT, "oracle", "flop_model.json")) as f:
-            ch = json.load(f)["channel_step"][3]
+            ch = json.load(f)["channel_step_order6" if args.visc_order == 6 else "channel_step"][3]
         fm = {k: v * ch / fm["step"] for k, v in fm.items()}   # pieces scaled like the Taylor-Green split
     # roofline of the dominant kernel (bound: plain FP64/FP32 ALUs; nothing here is a contraction).  The step kernels
     # are timed inside a long run, so the sustained peak is the roofline's; the burst figure is reported beside it.
@@ -405,8 +410,9 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": ("channel 192x128x128 (BASELINE.json configs[2]: isothermal walls, Sutherland, body force, tanh y grid; "
-                                "jf_cfl_dt_dev + jf_rk3_step_dev every step)") if channel else
-                               f"tgv{n} {'fp64' if args.dtype == 'f64' else 'fp32'} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)",
+                                "jf_cfl_dt_dev + jf_rk3_step_dev every step)" + (", sixth-order central dissipative flux" if args.visc_order == 6 else "")) if channel else
+                               f"tgv{n} {'fp64' if args.dtype == 'f64' else 'fp32'} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)"
+                               + (" [sixth-order dissipative flux; flops counted for the fourth-order scheme]" if args.visc_order == 6 else ""),
                    "cells": cells, "state_bytes": state_bytes, "l2": "inputs larger than L2 (no flush)" if state_bytes > 126e6 else "state fits L2",
                    "parallelism": f"replicas x{world}" if world > 1 else "1 GPU", "finite": finite,
                    "launch": "CUDA graph of the 15 kernels of a step, replayed (+ 1 one-thread kernel carrying a host dt)"},
@@ -436,7 +442,7 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: one RK3 step of the SAME input on the host cores (the oracle as it stands)
         nb = min(n, 256)
-        val, secs, cores = oracle_throughput(nb, 1, 0, channel)
+        val, secs, cores = oracle_throughput(nb, 1, 0, channel, args.visc_order)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": (f"1 step (cfl_dt + RK3) of the channel 192x128x128 fp64 ({secs:.1f} s)" if channel
                                            else f"1 RK3 step of tgv{nb} fp64 ({secs:.1f} s)")}

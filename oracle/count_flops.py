@@ -42,6 +42,11 @@ def main():
     model["channel_step"] = (o.count_flops_step(o.state(), 1e-4) / c.cells).tolist()
     model["channel_dims"] = list(c.n)
     print("channel flops per cell-step:", model["channel_step"][3], flush=True)
+    # the same step with the sixth-order dissipative flux (jf_set_visc_order(6))
+    c.visc_order = 6
+    o = ora.Oracle(c)
+    model["channel_step_order6"] = (o.count_flops_step(o.state(), 1e-4) / c.cells).tolist()
+    print("channel flops per cell-step, sixth-order dissipative flux:", model["channel_step_order6"][3], flush=True)
     with open(os.path.join(ROOT, "oracle", "flop_model.json"), "w") as f:
         json.dump(model, f, indent=1)
     print("asymptotic flops per cell-step:", model["step"][3][0])

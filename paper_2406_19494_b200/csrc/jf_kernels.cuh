@@ -1,14 +1,20 @@
-// jf_kernels.cuh — the CUDA kernels of libjf (sm_100a), templated on the scalar type.
+// jf_kernels.cuh — the CUDA kernels of libjf (sm_100a), templated on the scalar type (double, float, jf::Dual).
 //
-//   halo_kernel<AXIS>       a1  halo / boundary fill (Eq. 8)
-//   gradient_kernel         a5  nine 4th-order centre derivatives of (u,v,w) (transverse part of Eq. 5)
-//   sweep_x_kernel          a2-a6 along x: one warp per grid line, 32-face chunks, primitives in a
-//                           warp-private shared-memory ring, flux differences by warp shuffle
-//   sweep_yz_kernel<DIR>    a2-a6 along y / z: one thread per (x, other) column marching along
-//                           DIR (warp = 32 consecutive x: every access coalesced), 6-cell primitive
-//                           window in a thread-private shared-memory ring; the z sweep fuses the
-//                           source term and the SSP-RK3 stage update (a7)
-//   cfl_kernel              a8  warp-shuffle min reduction
+//   halo_all_kernel         a1  halo / boundary fill (Eq. 8): the x -> y -> z passes composed
+//                           per ghost cell in ONE launch; halo_kernel<AXIS> is one pass (decomposed blocks)
+//   face_xfer_kernel        a1 across blocks: pack / unpack / pull of an inter-block face
+//   gradient_kernel         a5  (part) the nine 4th-order centre derivatives of (u,v,w): plane march over an (x,y)
+//                           tile, double-buffered shared-memory planes, z derivative from a register queue
+//                           (gradient6_kernel: 6th order; jf_tma.cuh: the TMA-staged variant)
+//   sweep_x_kernel          a2-a6 along x: one warp per group of 4 lines swept as ONE stream of cells, lane = cell,
+//                           per-cell WENO, W^- and the face flux handed to the next lane by shuffle, primitives in
+//                           a warp-private 64-cell shared-memory ring
+//   sweep_yz_kernel<DIR>    a2-a6 along y / z: one thread per (x, other) column marching along DIR (warp = 32
+//                           consecutive x: every access coalesced), 5-cell (6 for the 6th-order dissipative flux)
+//                           window of 10 values in a thread-private shared-memory ring; the z sweep fuses the source
+//                           term and the SSP-RK3 stage update (a7), dt from a kernel argument or from device memory
+//   cfl_kernel              a8  warp-shuffle min reduction, ordered-bits atomicMin; optionally finished on the device
+//   plane_sums_kernel       plane statistics
 //
 // Data layout in HBM: SoA U[5][Pz][Py][Px] (x fastest), Nh = 3 halo layers.
 #pragma once
@@ -21,7 +27,9 @@ constexpr int NH = 3;
 
 // Tangent type (value, tangent): twice the registers per value.  The marching sweeps hold 100 KB of window per block,
 // so two blocks per SM is all that fits in shared memory anyway: give them the 255 registers that leaves (at the
-// primal's 168 they spilled 450-650 bytes per thread); the x sweep likewise runs 2 blocks of 4 warps at 255.
+// primal's 168 they spilled 450-650 bytes per thread); the x sweep likewise runs 2 blocks of 4 warps at 255.  The
+// gradient pass keeps ONE block per SM at 255 registers: at two blocks (128 registers) it spills 160 bytes and
+// takes 2.48 instead of 1.32 ms per step at 192^3.  Tangent step / primal step: 3.7-3.9 before, 2.6-2.65 now.
 #ifndef JF_XS_MINB_DUAL
 #define JF_XS_MINB_DUAL 2
 #endif
@@ -29,7 +37,7 @@ constexpr int NH = 3;
 #define JF_YZ_MINB_DUAL 2
 #endif
 #ifndef JF_GM_MINB_DUAL
-#define JF_GM_MINB_DUAL 2
+#define JF_GM_MINB_DUAL 1
 #endif
 
 template <class T>
