@@ -35,7 +35,9 @@ def parse_args():
     ap.add_argument("--case", default="tgv", choices=["tgv", "channel"],
                     help="tgv: BASELINE.json configs[4] (default, the metric's workload); channel: configs[2] "
                          "(192x128x128, walls, Sutherland, body force, CFL time step taken every step)")
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32", "f64t"],
+                    help="f64t: the tangent solver (JF_F64_TANGENT: value + derivative w.r.t. the disturbance-wall parameters); "
+                         "its roofline fields use the primal's flop count and fp64 peak (the tangent part is not counted)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-size", type=int, default=96, help="n^3 sample the reference arm steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -252,7 +254,7 @@ def run_ours(args):
     case = cases.channel() if channel else cases.tgv(n)
     case.visc_order = args.visc_order
     solver = jf.Solver(case, args.dtype, device=str(dev))
-    esz = 8 if args.dtype == "f64" else 4
+    esz = {"f64": 8, "f32": 4, "f64t": 16}[args.dtype]
     U = solver.state()
     dt = case.dt
     state_bytes = U.numel() * esz
@@ -284,7 +286,7 @@ def run_ours(args):
     ktimes = solver.jf_diag_kernel_times()
     solver.jf_diag_timing(False)
     clk = clocks.stop()
-    finite = bool(torch.isfinite(U).all().item())
+    finite = solver.jf_cfl_dt(U, 1.0)[0] == 0          # the library's own reduction: every interior cell finite, rho, p > 0
 
     # --- end to end: host buffers, H2D of the input and D2H of the result inside every step.  Every step is one
     # independent job (its own input from pinned host memory, its own result back in pinned host memory); the jobs
@@ -293,7 +295,7 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         host_in = torch.empty(U.shape, dtype=U.dtype, pin_memory=True)
-        host_in.copy_(torch.as_tensor(case.U0, dtype=U.dtype))
+        host_in.copy_(solver.state().cpu() if args.dtype == "f64t" else torch.as_tensor(case.U0, dtype=U.dtype))
         host_out = [torch.empty(U.shape, dtype=U.dtype, pin_memory=True) for _ in range(2)]
         bufs = [U, torch.empty_like(U)]
         cur = torch.cuda.current_stream(dev)
@@ -349,7 +351,7 @@ def run_ours(args):
             sclk = sck.stop()
             sweep.append({"size": sn, "dtype": sdt, "cells": sc.cells, "steps": 5, "ms_per_step": sms / 5,
                           "value": sc.cells * 5 / (sms * 1e-3), "sm_mhz": sclk.get("sm_mhz"), "reasons": sclk.get("reasons"),
-                          "finite": bool(torch.isfinite(SU).all().item())})
+                          "finite": ss.jf_cfl_dt(SU, 1.0)[0] == 0})
             del ss, SU
             torch.cuda.empty_cache()
 
@@ -373,7 +375,8 @@ def run_ours(args):
     # are timed inside a long run, so the sustained peak is the roofline's; the burst figure is reported beside it.
     # The peak loop holds the maximum SM clock while the step runs into the board's power cap, so the fraction at the
     # clock the step actually ran at is reported too (peak scaled by run clock / peak-loop clock).
-    peak_burst, peak_flops, peak_mhz = alu_peak(jf, args.dtype, local)
+    pdt = "f32" if args.dtype == "f32" else "f64"
+    peak_burst, peak_flops, peak_mhz = alu_peak(jf, pdt, local)
     run_mhz = clk.get("sm_mhz")
     clock_ratio = (run_mhz / peak_mhz) if (run_mhz and peak_mhz) else None
     sweep_flops = (fm["rhs"] - fm["prim"] - fm["grad"]) / 3.0           # one direction: WENO5+HLLC+viscous face+divergence
@@ -387,6 +390,7 @@ def run_ours(args):
     achieved = dom_flops / dom_s / 1e12 if dom_n else 0.0
     # measured DRAM bytes and executed FP64 instructions of the dominant kernel (committed ncu capture)
     row = None if channel else profile_row(dom, n, args.dtype)
+    bdt = "f32" if args.dtype == "f32" else "f64"       # bytes / flops model of the value part
     traffic = float(row["dram_bytes_per_launch"]) if row else None
     executed = None
     if row and row.get("dfma_thread_inst"):
@@ -396,7 +400,7 @@ def run_ours(args):
                                  "divisions / square roots appear as the Newton steps they are executed as)"}
     peaks = measured_peaks()
     hbm = peaks.get("hbm_gbs", 6650.0)
-    troof = t_roof_ms(fm["step"], cells, args.dtype, peak_flops, hbm)
+    troof = t_roof_ms(fm["step"], cells, bdt, peak_flops, hbm)
     if sweep:
         for ln in sweep:
             sfm = flop_model(ln["size"])
@@ -411,7 +415,7 @@ def run_ours(args):
         "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": ("channel 192x128x128 (BASELINE.json configs[2]: isothermal walls, Sutherland, body force, tanh y grid; "
                                 "jf_cfl_dt_dev + jf_rk3_step_dev every step)" + (", sixth-order central dissipative flux" if args.visc_order == 6 else "")) if channel else
-                               f"tgv{n} {'fp64' if args.dtype == 'f64' else 'fp32'} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)"
+                               f"tgv{n} {dict(f64='fp64', f32='fp32', f64t='fp64 tangent solver')[args.dtype]} (BASELINE.json configs[4]: Taylor-Green {n}^3, dt=1e-3)"
                                + (" [sixth-order dissipative flux; flops counted for the fourth-order scheme]" if args.visc_order == 6 else ""),
                    "cells": cells, "state_bytes": state_bytes, "l2": "inputs larger than L2 (no flush)" if state_bytes > 126e6 else "state fits L2",
                    "parallelism": f"replicas x{world}" if world > 1 else "1 GPU", "finite": finite,
@@ -429,7 +433,7 @@ def run_ours(args):
                      "flops_per_cell_launch": alg.get(dom), "avg_launch_ms": dom_ms / dom_n if dom_n else None},
         "roofline_step": {"flops_per_cell_step": fm["step"], "t_roof_ms": troof, "frac": troof / (ms / K),
                           "frac_at_run_clock": troof / (ms / K) / clock_ratio if clock_ratio else None,
-                          "frac_of_burst_peak": t_roof_ms(fm["step"], cells, args.dtype, peak_burst, hbm) / (ms / K),
+                          "frac_of_burst_peak": t_roof_ms(fm["step"], cells, bdt, peak_burst, hbm) / (ms / K),
                           "hbm_gbs": hbm, "hbm_source": "measured" if peaks else "fallback"},
         "kernels_ms_per_step": {k: v[0] / K for k, v in ktimes.items() if v[1]},
     }
@@ -472,7 +476,7 @@ def run_decomp(args, torch, dist, jf, cases, world, rank, local, dev, barrier):
     clocks = ClockSampler(local)
     ms = time_steps(torch, lambda: rb.jf_rk3_step(dt), K, W, barrier, clocks)
     clk = clocks.stop()
-    finite = bool(torch.isfinite(rb.U).all().item())
+    finite = rb.jf_cfl_dt(1.0)[0] == 0
     (ms,) = max_over_ranks([ms], world, dev)
     if rank == 0:
         cells = part.case.cells

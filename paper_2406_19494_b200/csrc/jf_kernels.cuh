@@ -438,21 +438,47 @@ gradient6_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz
 #pragma unroll
   for (int a = 0; a < 7; ++a) q[a][0] = q[a][1] = q[a][2] = T(0);
   const int pstart = max(k0 - 3, 0), pend = min(k1 + 2, Pz - 1);
-  constexpr int NCELL = G6_SX * G6_SY, NTHR = GM_TX * GM_TY;
+  constexpr int NCELL = G6_SX * G6_SY, NTHR = GM_TX * GM_TY, NR = (NCELL + NTHR - 1) / NTHR;
+  // the cells of the plane this thread converts: in-plane offsets fixed over the march, raw values of the NEXT plane
+  // in flight while the current one is processed
+  unsigned off[NR];
+  bool in[NR];
+  int sidx[NR];
+  T nxt[NR][4];
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    const int c = tid + r * NTHR;
+    const int cy = c / G6_SX, cx = c - cy * G6_SX;
+    const int gx = x0 - 3 + cx, gy = y0 - 3 + cy;
+    in[r] = c < NCELL && gx >= 0 && gx < Px && gy >= 0 && gy < Py;
+    off[r] = (unsigned)gy * (unsigned)P.sy + (unsigned)gx;
+    sidx[r] = c < NCELL ? cy * G6_SX + cx : -1;
+  }
+  auto fetch = [&](int p) {
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+      const unsigned o = off[r] + (unsigned)p * sz;
+      nxt[r][0] = in[r] ? U[o] : T(1);
+      nxt[r][1] = in[r] ? (U + P.vol)[o] : T(0);
+      nxt[r][2] = in[r] ? (U + 2 * P.vol)[o] : T(0);
+      nxt[r][3] = in[r] ? (U + 3 * P.vol)[o] : T(0);
+    }
+  };
+  fetch(pstart);
   for (int p = pstart; p <= pend; ++p) {
     const int b = p & 1;
+    T cur[NR][4];
 #pragma unroll
-    for (int r = 0; r < (NCELL + NTHR - 1) / NTHR; ++r) {
-      const int c = tid + r * NTHR;
-      if (c < NCELL) {
-        const int cy = c / G6_SX, cx = c - cy * G6_SX;
-        const int gx = x0 - 3 + cx, gy = y0 - 3 + cy;
-        const bool in = gx >= 0 && gx < Px && gy >= 0 && gy < Py;
-        const unsigned o = (unsigned)gy * (unsigned)P.sy + (unsigned)gx + (unsigned)p * sz;
-        const T ri = Num<T>::rcp(in ? U[o] : T(1));
-        sv[b][0][cy][cx] = in ? (U + P.vol)[o] * ri : T(0);
-        sv[b][1][cy][cx] = in ? (U + 2 * P.vol)[o] * ri : T(0);
-        sv[b][2][cy][cx] = in ? (U + 3 * P.vol)[o] * ri : T(0);
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) cur[r][i] = nxt[r][i];
+    if (p < pend) fetch(p + 1);
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+      if (sidx[r] >= 0) {
+        const T ri = Num<T>::rcp(cur[r][0]);
+        T* d = &sv[b][0][0][0] + sidx[r];
+        d[0] = cur[r][1] * ri; d[NCELL] = cur[r][2] * ri; d[2 * NCELL] = cur[r][3] * ri;
       }
     }
     __syncthreads();
@@ -778,6 +804,11 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   // metric table entries of the face / cell the NEXT step treats, loaded one step ahead (a per-step
   // scalar load issued where it is used stalls the warp for an L2 round trip: 11-13 % of all stall samples)
   T xf_n = VISC ? P.i24Xf[DIR][c0 - 1 + NH - 1] : T(0), idl_n = P.inv_dl[DIR][c0 - 1 + NH - 1];
+#ifdef JF_YZ_UNROLL
+#define JF_PRAGMA_(x) _Pragma(#x)
+#define JF_PRAGMA(x) JF_PRAGMA_(x)
+  JF_PRAGMA(unroll JF_YZ_UNROLL)
+#endif
   for (int c = c0 - 1; c <= c1; ++c) {
     const int pc = c + NH;
     const T xf_c = xf_n, idl_c = idl_n;      // 1/(24 X_xi^f) of face c-1/2, 1/Delta of cell c-1
