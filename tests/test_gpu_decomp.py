@@ -32,12 +32,19 @@ def wall_case(n=(24, 12, 8)):
     return c
 
 
+def channel_sixth():
+    c = cases.channel(48, 32, 32, n_steps=3)
+    c.visc_order = 6                                          # the sixth-order dissipative flux reads cells -3..2 about a
+    return c                                                  # face: the same three exchanged layers suffice
+
+
 CASES = {
     "periodic": (lambda: cases.random_admissible(n=(24, 16, 12), seed=7, stretched=True), (2, 2, 2)),
     "periodic3x": (lambda: cases.random_admissible(n=(27, 9, 8), seed=8, stretched=True), (3, 1, 2)),
     "walls": (wall_case, (3, 2, 2)),
     "channel": (lambda: cases.channel(48, 32, 32, n_steps=3), (2, 2, 1)),
     "plate": (lambda: cases.flat_plate(256, 32, 8, n_steps=3), (4, 1, 1)),
+    "channel_order6": (channel_sixth, (2, 2, 2)),
 }
 
 

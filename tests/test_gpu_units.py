@@ -150,3 +150,29 @@ def test_geometry_tables_against_the_oracles(jf, ora, name, dtype):
             assert np.max(np.abs(i12Xc[ci] * 12.0 * Xc[ci] - 1.0)) <= 4 * tol
             fi = slice(2, n + 3)                          # X_xi^f: faces -1/2 .. n-1/2
             assert np.max(np.abs(i24Xf[fi] * 24.0 * Xf[fi] - 1.0)) <= 4 * tol
+
+
+def test_bench_line_schema_on_a_small_box(jf):
+    # the one JSON line bench.py prints, through the real GPU path on a 48^3 box: the contract's keys and the
+    # tier's additions (roofline with both numerators and both clocks, cpu_baseline, e2e with host copies)
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--size", "48", "--steps", "3", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+              "dtype", "data", "config", "clocks", "gpu_launches", "roofline", "roofline_step", "e2e", "cpu_baseline"):
+        assert k in d, k
+    assert d["unit"] == "cell-updates/s" and d["dtype"] == "f64" and d["steps"] == 3 and d["vs_baseline"] is None
+    assert d["gpu_launches"] == 3 * 16 and d["config"]["finite"] is True
+    r = d["roofline"]
+    assert r["bound"] == "alu" and 0 < r["frac"] < 1 and r["peak"] > 20 and "numerator" in r and "frac_at_run_clock" in r
+    assert d["e2e"]["h2d_bytes_per_step"] == d["config"]["state_bytes"] == 5 * 54 ** 3 * 8 and d["e2e"]["value"] < d["value"]
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
+    assert d["value"] == pytest.approx(48 ** 3 * 3 / (d["ms_per_step"] * 3 * 1e-3), rel=1e-9)
