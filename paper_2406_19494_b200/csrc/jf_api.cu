@@ -1039,6 +1039,10 @@ jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {
   if (s->dtype != JF_F64_TANGENT) return fail(s, JF_EINVAL, "jf_set_tangent_seed: not a tangent solver");
   if (!(dA == dA) || !(dkappa == dkappa)) return fail(s, JF_EINVAL, "jf_set_tangent_seed: NaN seed");
   for (int f = 0; f < 6; ++f) { s->t.bc[f].dA = dA; s->t.bc[f].dkappa = dkappa; }
+  // the halo kernels take the face tables by value: captured steps would replay the old seed
+  JF_CUDA(s, cudaStreamSynchronize(s->stream));
+  for (auto& g : s->graphs) cudaGraphExecDestroy(g.exec);
+  s->graphs.clear();
   return JF_OK;
 }
 

@@ -194,3 +194,27 @@ def test_seed_rejected_on_plain_solvers(jf):
     s = jf.Solver(c, "f64")
     with pytest.raises(jf.JFError):
         s.jf_set_tangent_seed(1.0, 0.0)
+
+
+def test_changing_the_seed_on_a_live_solver_takes_effect(jf):
+    # the step is replayed from a CUDA graph whose halo kernels carry the face tables by value: a new seed must
+    # invalidate the captured steps.  Linear in the seed: the tangent after steps with seed (2, 0) from a zero
+    # tangent is twice the one with seed (1, 0), on the same solver and the same state array.
+    import torch
+    c = wall_case()
+    s = jf.Solver(c, "f64t")
+    U = s.state()
+    U0 = U.clone()
+    s.jf_set_tangent_seed(1.0, 0.0)
+    for _ in range(2):
+        s.jf_rk3_step(U, 1e-3)
+    t1 = U[..., 1].clone()
+    U.copy_(U0)
+    s.jf_set_tangent_seed(2.0, 0.0)
+    for _ in range(2):
+        s.jf_rk3_step(U, 1e-3)
+    torch.cuda.synchronize()
+    t2 = U[..., 1]
+    scale = float(t1.abs().max())
+    assert scale > 0
+    assert float((t2 - 2.0 * t1).abs().max()) <= 1e-12 * scale
