@@ -11,6 +11,8 @@
 #include "../../include/jf.h"
 #include "jf_kernels.cuh"
 #include "jf_tma.cuh"
+#include "jf_pc.cuh"
+#include <type_traits>
 #include <cstdlib>
 #include <unordered_map>
 
@@ -151,6 +153,7 @@ struct jf_solver {
   char* ws = nullptr;
   // TMA-staged gradient pass (jf_tma.cuh): tensor maps per state-array base address (U, stage buffers A, B, ...)
   bool grad_tma = false;
+  bool yz_pc = false;            // producer / consumer form of the marching sweeps (jf_pc.cuh; fp64, viscous, fourth order)
   std::unordered_map<const void*, CUtensorMap> maps;
   // CUDA graphs of one RK3 step (the 15 launches), one per state-array address, captured on first use on a private
   // stream and launched into the caller's stream.  The kernels of a graph read dt from the device scalar
@@ -519,9 +522,30 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
     const size_t sh = (size_t)jf::XS_WARPS * (jf::XS<VISC>::NV * jf::XS_RING + jf::XS_CARRY) * sizeof(T);
     jf::sweep_x_kernel<T, VISC, ORD><<<(groups + jf::XS_WARPS - 1) / jf::XS_WARPS, jf::XS_WARPS * 32, sh, s->stream>>>(P, U, G, R);
   }
+  jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0), nullptr};
+  if constexpr (std::is_same<T, double>::value && VISC && ORD == 4) {
+    if (s->yz_pc) {
+      const size_t shp = jf::pc_smem_bytes();
+      {
+        Timed t(s, K_SWEEP_Y);
+        const int L = s->seg_len[1];
+        dim3 grid((P.n[0] + 31) / 32, (P.n[2] + 3) / 4, (P.n[1] + L - 1) / L);
+        jf::sweep_yz_pc_kernel<1, 0><<<grid, 256, shp, s->stream>>>(P, U, G, R, none, L);
+      }
+      {
+        Timed t(s, K_SWEEP_Z);
+        const int L = s->seg_len[2];
+        dim3 grid((P.n[0] + 31) / 32, (P.n[1] + 3) / 4, (P.n[2] + L - 1) / L);
+        if (rk) jf::sweep_yz_pc_kernel<2, 2><<<grid, 256, shp, s->stream>>>(P, U, G, R, *rk, L);
+        else jf::sweep_yz_pc_kernel<2, 1><<<grid, 256, shp, s->stream>>>(P, U, G, R, none, L);
+      }
+      s->launches += 3;
+      JF_CUDA(s, cudaPeekAtLastError());
+      return JF_OK;
+    }
+  }
   const size_t sh = jf::yz_smem_bytes<T, VISC, ORD>();
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
-  jf::RKArgs<T> none{nullptr, nullptr, T(0), T(0), T(0), nullptr};
   {
     Timed t(s, K_SWEEP_Y);
     const int L = s->seg_len[1];
@@ -805,6 +829,21 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
     }
   }
   if (const char* e = std::getenv("JF_GRAPH")) s->use_graph = std::atoi(e) != 0;
+  {
+    bool want = false;
+#ifdef JF_YZ_PC_DEFAULT
+    want = JF_YZ_PC_DEFAULT != 0;
+#endif
+    if (const char* e = std::getenv("JF_YZ_PC")) want = std::atoi(e) != 0;
+    s->yz_pc = want && dtype == JF_F64 && s->viscous;
+    if (s->yz_pc) {
+      const int shp = (int)jf::pc_smem_bytes();
+      cudaError_t ce = cudaFuncSetAttribute((const void*)jf::sweep_yz_pc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, shp);
+      if (ce == cudaSuccess) ce = cudaFuncSetAttribute((const void*)jf::sweep_yz_pc_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, shp);
+      if (ce == cudaSuccess) ce = cudaFuncSetAttribute((const void*)jf::sweep_yz_pc_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, shp);
+      if (ce != cudaSuccess) s->yz_pc = false;
+    }
+  }
   const int n[3] = {g->nx, g->ny, g->nz};
   s->seg_len[0] = 0;
   auto cdiv = [](int a, int b) { return (long long)((a + b - 1) / b); };

@@ -524,6 +524,34 @@ def test_graph_replay_is_bitwise_the_plain_launch_sequence(jf, name):
     assert Va.cpu().numpy().tobytes() == Vb.cpu().numpy().tobytes()
 
 
+@pytest.mark.parametrize("variant", ["JF_YZ_PC", "JF_GRAD_TMA"])
+@pytest.mark.parametrize("name", ["ragged", "bc0", "bc1", "tiny", "channel"])
+def test_selectable_kernel_variants_against_the_oracle(jf, ora, variant, name):
+    # the measured-and-not-adopted variants stay selectable: the producer / consumer form of the
+    # marching sweeps (jf_pc.cuh) and the TMA-staged gradient pass (jf_tma.cuh).  Same parity bar as the default path.
+    import os
+    c = {"ragged": lambda: cases.random_admissible(n=(70, 35, 67), seed=9, stretched=True),
+         "bc0": lambda: all_bc_case(n=(38, 21, 13), which=0), "bc1": lambda: all_bc_case(n=(38, 21, 13), which=1),
+         "tiny": lambda: cases.random_admissible(n=(4, 4, 4), seed=10), "channel": lambda: cases.channel(48, 32, 32, n_steps=20)}[name]()
+    c.body_accel = (0.3, -0.2, 0.1) if name.startswith("bc") else c.body_accel
+    os.environ[variant] = "1"
+    try:
+        s = jf.Solver(c, "f64")
+    finally:
+        del os.environ[variant]
+    o = ora.Oracle(c, "f64")
+    Ro = o.rhs(o.fill_halo(o.state()))
+    R = s.jf_rhs(s.jf_fill_halo(s.state())).cpu().numpy()
+    assert np.all(metric_R(R, Ro) <= TOL["f64"])
+    n_steps = 20 if name == "channel" else 3
+    Uo, U = o.state(), s.state()
+    for _ in range(n_steps):
+        st, dt = o.cfl_dt(Uo, 0.5)
+        o.rk3_step(Uo, dt)
+        s.jf_rk3_step(U, dt)
+    assert np.all(metric_P(U.cpu().numpy(), Uo) <= TOL["f64"])
+
+
 @pytest.mark.parametrize("name", ["channel", "sod", "plate"])
 def test_device_resident_dt_equals_the_host_loop(jf, ora, name):
     # jf_cfl_dt_dev + jf_rk3_step_dev (the step is formed and consumed on the device, t_end clipping included)
