@@ -477,10 +477,6 @@ const CUtensorMap* grad_map(jf_solver* s, const jf::Params<T>& P, const T* U) {
   if (s->maps.size() > 64) s->maps.clear();
   return &(s->maps[(const void*)U] = m);
 }
-template <>
-const CUtensorMap* grad_map<jf::Dual>(jf_solver*, const jf::Params<jf::Dual>&, const jf::Dual*) { return nullptr; }
-template <>
-const CUtensorMap* grad_map<float>(jf_solver*, const jf::Params<float>&, const float*) { return nullptr; }
 
 template <class T>
 bool launch_grad_tma(jf_solver* s, Impl<T>& I, const T* U, dim3 grid, int Lz) {

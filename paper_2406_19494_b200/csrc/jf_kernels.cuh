@@ -782,10 +782,13 @@ sweep_yz_kernel(Params<T> P, const T* __restrict__ U, const T* __restrict__ G, T
   // tangent type (four registers per value), through thread-private shared memory: variable q lives in the unused
   // tenth value of ring slot q.  (For fp64 the exchange was measured, also with 4 blocks per SM at 128 registers,
   // which it makes spill-free: y 1.91 -> 1.99 ms, z + RK 2.15 -> 2.21 ms per step at 256^3; not used there.)
+#ifndef JF_YZ_XCHG_MASK
+#define JF_YZ_XCHG_MASK 0
+#endif
 #ifdef JF_YZ_XCHG
   constexpr bool XCHG = true;
 #else
-  constexpr bool XCHG = sizeof(T) > 8;
+  constexpr bool XCHG = sizeof(T) > 8 || ((JF_YZ_XCHG_MASK >> MODE) & 1);
 #endif
   auto xw = [&](int q) -> T* {
     if (PAIR) return &(mine + q * (NP * NT) + (NP - 1) * NT)->b;

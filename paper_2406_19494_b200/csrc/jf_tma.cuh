@@ -62,8 +62,8 @@ struct GradTmaSmem {
 template <class T>
 __global__ void __launch_bounds__(GM_TX * GM_TY, 3)
 gradient_tma_kernel(Params<T> P, const __grid_constant__ CUtensorMap mapU, T* __restrict__ G, int Lz) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  GradTmaSmem<T>& S = *reinterpret_cast<GradTmaSmem<T>*>(smem_raw);
+  extern __shared__ __align__(128) unsigned char smem_tma[];
+  GradTmaSmem<T>& S = *reinterpret_cast<GradTmaSmem<T>*>(smem_tma);
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * GM_TX + tx;
   const int x0 = blockIdx.x * GM_TX, y0 = blockIdx.y * GM_TY;
   const int px = x0 + tx, py = y0 + ty;
