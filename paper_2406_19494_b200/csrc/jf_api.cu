@@ -665,8 +665,9 @@ jf_status rk3(jf_solver* s, Impl<T>& I, T* U, double dt, bool dev_dt) {
 
 template <class T>
 int cfl_blocks(const Impl<T>& I) {
-  const long long ncell = (long long)I.P.n[0] * I.P.n[1] * I.P.n[2];
-  return (int)std::min<long long>((ncell + 255) / 256, 148LL * 8);
+  // one warp per 32-cell chunk of a grid line; at most 8 resident blocks of 8 warps on each of the 148 SMs
+  const long long ntask = (long long)((I.P.n[0] + 31) / 32) * I.P.n[1] * I.P.n[2];
+  return (int)std::max<long long>(1, std::min<long long>((ntask + 7) / 8, 148LL * 8));
 }
 
 // reduction + finalize on the device (no host synchronisation): dt -> cfl_out[5], t += dt -> cfl_out[6]
