@@ -51,7 +51,10 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, u
 // cell once, 1.7 cells per thread); __syncthreads; the elected thread re-arms the slot the previous plane used and
 // issues the box of plane p + NS - 1; every thread forms the x / y derivatives of its cell from the shared plane and
 // the z derivative of the plane two steps back from a five-deep register queue of its own cell.
-constexpr int GT_NS = 3;
+#ifndef JF_GT_NS
+#define JF_GT_NS 3
+#endif
+constexpr int GT_NS = JF_GT_NS;
 template <class T>
 struct GradTmaSmem {
   alignas(128) T raw[GT_NS][4][GM_SY][GM_SX];
