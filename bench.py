@@ -470,6 +470,10 @@ def run_decomp(args, torch, dist, jf, cases, world, rank, local, dev, barrier):
     if len(S) != 3 or S[0] * S[1] * S[2] != world:
         raise SystemExit(f"bench.py --decomp {args.decomp}: needs {S[0] * S[1] * S[2] if len(S) == 3 else '?'} ranks, have {world}")
     n, K, W = args.size, args.steps, max(args.warmup, 3)
+    if world == 1 and not dist.is_initialized():       # a single block: the arm still goes through RankBlock (no exchange faces)
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
     part = decomp.tgv_part(n, S, rank)
     rb = decomp.RankBlock(None, S, args.dtype, device=str(dev), part=part)
     dt = part.case.dt
@@ -492,7 +496,7 @@ def run_decomp(args, torch, dist, jf, cases, world, rank, local, dev, barrier):
                         "dof_cells": pid_seconds(ms / K, world, cells * world),
                         "dof_cells_x5": pid_seconds(ms / K, world, 5 * cells * world), "unit": "s"}}
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 

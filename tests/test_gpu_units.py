@@ -176,3 +176,23 @@ def test_bench_line_schema_on_a_small_box(jf):
     assert d["e2e"]["h2d_bytes_per_step"] == d["config"]["state_bytes"] == 5 * 54 ** 3 * 8 and d["e2e"]["value"] < d["value"]
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
     assert d["value"] == pytest.approx(48 ** 3 * 3 / (d["ms_per_step"] * 3 * 1e-3), rel=1e-9)
+
+
+def test_decomposition_arm_of_bench_on_one_rank(jf):
+    # bench.py --decomp with a single block: the arm's whole code path (RankBlock over torch.distributed, axis-by-axis halo
+    # passes, stage calls, max-over-ranks timing, PID of Eq. 9) except the exchange itself, which needs a second GPU
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MASTER_PORT="29541")
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--decomp", "1,1,1", "--size", "48", "--steps", "4"],
+                         capture_output=True, text=True, timeout=600, env=env)
+    assert out.returncode == 0, out.stderr[-3000:]
+    d = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+    assert d["n_gpus"] == 1 and d["scaling"] == "weak" and d["config"]["finite"] is True
+    assert d["config"]["exchange_bytes_per_rank_per_step"] == 0
+    assert d["gpu_launches"] == 4 * 3 * 7                     # per stage: three axis passes, gradient, x, y, z + RK
+    assert d["pid"]["dof_cells"] == pytest.approx(d["ms_per_step"] * 1e-3 / 48 ** 3, rel=1e-9)
+    assert d["pid"]["dof_cells_x5"] == pytest.approx(d["pid"]["dof_cells"] / 5, rel=1e-12)
