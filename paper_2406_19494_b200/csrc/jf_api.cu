@@ -1133,6 +1133,6 @@ jf_status jf_diag_metrics(jf_solver* s, int axis, double* inv_delta, double* cen
                      diag_metrics<jf::Dual>(s, s->t, axis, inv_delta, centre, i12Xc, i24Xf));
 }
 
-const char* jf_version(void) { return "libjf 0.1 (sm_100a; WENO5-JS + HLLC + 4th-order viscous + SSP-RK3)"; }
+const char* jf_version(void) { return "libjf 0.2 (sm_100a; WENO5-JS + HLLC + 4th- or 6th-order central viscous flux + SSP-RK3; CUDA-graph step, device-resident dt)"; }
 
 }  // extern "C"
