@@ -163,7 +163,14 @@ jf_status jf_dev_time(jf_solver *s, int set, double *dt_host, double *t_host);
 /* Launch mechanics of jf_rk3_step / jf_rk3_step_dev: the 15 launches of a step are captured once per state-array
  * address into a CUDA graph owned by the solver (on a private stream) and replayed into the caller's stream; their
  * z + RK kernels read dt from the device scalar, which jf_rk3_step sets with a one-thread kernel.  Environment
- * JF_GRAPH=0 at jf_create time turns this off (plain launches; also used while jf_diag_timing is on). */
+ * JF_GRAPH=0 at jf_create time turns this off (plain launches; also used while jf_diag_timing is on).
+ *
+ * Environment variables read once, at jf_create (tuning / A-B measurements; none changes a result beyond round-off):
+ *   JF_GRAPH=0      plain launches instead of the CUDA-graph replay
+ *   JF_GRAD_TMA=1   TMA-staged centre-gradient pass (cp.async.bulk.tensor + mbarrier ring; fp64, even nx): 6 % faster at
+ *                   256^3, 22 % slower at 512^3, hence not the default (profiles/r2_tma_sass.md)
+ *   JF_YZ_PC=1      producer / consumer form of the y / z sweeps (fp64, viscous, fourth-order flux): 20 % slower, kept as a
+ *                   measured variant (profiles/r2_experiments.md) */
 
 /* ---- Block decomposition ------------------------------------------
  * One solver per block; faces between blocks are JF_BC_EXCHANGE.  One RK stage of a decomposed step is
