@@ -222,6 +222,21 @@ jf_status jf_rk3_stage_advance(jf_solver *s, void *U_dev, int stage, double dt);
 #define JF_NSTATS 14
 jf_status jf_plane_sums(jf_solver *s, const void *U_dev, int axis, double *sums_dev);
 
+/* jf_plane_sums for callers that must not allocate and have no workspace to spare for it (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the same two kernels and the same summation
+ * order (the same bits as jf_plane_sums), but the per-block partial sums go to a STATIC device array inside the
+ * library (14 x 1024 x 16 doubles = 1.75 MiB per GPU that loads the library, held until the process exits) instead of
+ * the solver's workspace.  The call allocates nothing on host or device (no cudaMalloc / cudaFree, no allocating
+ * library routine; the array's device address is looked up once per device with cudaGetSymbolAddress and cached).
+ * Limit: at most jf_plane_sums_static_max_planes() = 1024 interior planes along `axis`; larger grids get JF_EINVAL
+ * with the reason in jf_last_error (use jf_plane_sums).  sums_dev as for jf_plane_sums (DEVICE, JF_NSTATS * n_axis
+ * doubles, caller-owned).  The array is shared by every solver and every call on that GPU and keeps the last call's
+ * contents; nothing in it needs clearing (each call writes every partial it reads), but two calls that OVERLAP on the
+ * GPU (different streams, no ordering between them) race on it: order them on one stream or with events.
+ * Asynchronous on the solver's stream. */
+jf_status jf_plane_sums_static(jf_solver *s, const void *U_dev, int axis, double *sums_dev);
+int jf_plane_sums_static_max_planes(void);
+
 /* Tangent solvers (JF_F64_TANGENT) only; JF_EINVAL otherwise.  The paper introduces the Disturbance
  * Wall so that its parameters can be differentiated through the solver.
  * Sets the direction (dA, dkappa) in the parameter space of Eq. 8 (:112), applied to every disturbance

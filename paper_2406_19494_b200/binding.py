@@ -47,7 +47,7 @@ class jf_bc(C.Structure):
 
 EXPORTS = ["jf_workspace_bytes", "jf_create", "jf_destroy", "jf_state_elems", "jf_fill_halo", "jf_rhs",
            "jf_rk3_step", "jf_cfl_dt", "jf_cfl_dt_dev", "jf_rk3_step_dev", "jf_dev_time", "jf_set_visc_order", "jf_set_tangent_seed", "jf_fill_halo_axis", "jf_face_elems", "jf_pack_face",
-           "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
+           "jf_unpack_face", "jf_pull_face", "jf_rk3_stage_input", "jf_rk3_stage_advance", "jf_plane_sums", "jf_plane_sums_static", "jf_plane_sums_static_max_planes", "jf_last_error", "jf_launch_count", "jf_diag_alu_peak", "jf_diag_timing",
            "jf_diag_kernel_times", "jf_diag_kernel_name", "jf_diag_face_flux", "jf_diag_metrics", "jf_version"]
 
 _lib = None
@@ -96,6 +96,10 @@ def lib():
         L.jf_rk3_stage_advance.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double]
         L.jf_plane_sums.restype = C.c_int
         L.jf_plane_sums.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.jf_plane_sums_static.restype = C.c_int
+        L.jf_plane_sums_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.jf_plane_sums_static_max_planes.restype = C.c_int
+        L.jf_plane_sums_static_max_planes.argtypes = []
         L.jf_set_tangent_seed.restype = C.c_int
         L.jf_set_tangent_seed.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.jf_rk3_step.restype = C.c_int
@@ -298,6 +302,14 @@ class Solver:
         """[JF_NSTATS = 14][n_axis] float64 device tensor of the area-weighted plane sums (include/jf.h)."""
         out = self.torch.empty((14, self.case.n[axis]), dtype=self.torch.float64, device=self.device)
         self._check(lib().jf_plane_sums(self.h, self._ptr(U), int(axis), C.c_void_p(out.data_ptr())))
+        return out
+
+    def jf_plane_sums_static(self, U, axis, out=None):
+        """jf_plane_sums through the library's static scratch array (allocation-free entry point, include/jf.h);
+        `out`: a preallocated [14, n_axis] float64 device tensor (allocated here if None)."""
+        if out is None:
+            out = self.torch.empty((14, self.case.n[axis]), dtype=self.torch.float64, device=self.device)
+        self._check(lib().jf_plane_sums_static(self.h, self._ptr(U), int(axis), C.c_void_p(out.data_ptr())))
         return out
 
     def jf_set_visc_order(self, order):

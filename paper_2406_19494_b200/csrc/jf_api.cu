@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -131,6 +132,39 @@ namespace {
 bool dtype_ok(jf_dtype d) { return d == JF_F64 || d == JF_F32 || d == JF_F64_TANGENT; }
 size_t elem_size(jf_dtype d) { return d == JF_F64 ? sizeof(double) : (d == JF_F32 ? sizeof(float) : sizeof(jf::Dual)); }
 
+}  // namespace
+
+// ---- scratch of the allocation-free entry point jf_plane_sums_static (include/jf.h) ----------------------------
+// Partial sums of plane_sums_kernel: NSTAT quantities x planes x STATS_NB partial blocks, for at most
+// JF_STATIC_MAX_PLANES planes: 14 x 1024 x 16 doubles = 1.75 MiB.  Lives in every GPU context that loads the library
+// until the process exits.  In HOST code the name `jf_static_scratch` is a host-side stand-in, not a device address:
+// host code takes the address once per device with cudaGetSymbolAddress (static_scratch_ptr below) and hands THAT to
+// the kernels.  All calls on one device share the array and it keeps the last call's contents; nothing in it has to
+// start at zero (every partial a call reads is written by that call first).
+#define JF_STATIC_MAX_PLANES 1024
+static __device__ __align__(256) double jf_static_scratch[(size_t)jf::NSTAT * JF_STATIC_MAX_PLANES * STATS_NB];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex static_scratch_mutex;
+double* static_scratch_addr[STATIC_MAX_DEVICES] = {};
+
+// Device address of jf_static_scratch on the CURRENT device; resolved once per device, then cached.
+cudaError_t static_scratch_ptr(double** out) {
+  int dev = -1;
+  cudaError_t ce = cudaGetDevice(&dev);
+  if (ce != cudaSuccess) return ce;
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(static_scratch_mutex);
+  if (!static_scratch_addr[dev]) {
+    double* ptr = nullptr;
+    ce = cudaGetSymbolAddress((void**)&ptr, jf_static_scratch);
+    if (ce != cudaSuccess) return ce;
+    static_scratch_addr[dev] = ptr;
+  }
+  *out = static_scratch_addr[dev];
+  return cudaSuccess;
+}
 }  // namespace
 
 struct jf_solver {
@@ -723,6 +757,32 @@ jf_status plane_sums(jf_solver* s, Impl<T>& I, const T* U, int axis, double* out
   return JF_OK;
 }
 
+// jf_plane_sums with the partial sums in the library's static device array instead of the caller's workspace: same
+// kernels, same launch configuration, same summation order => the same bits as plane_sums above.  Allocates nothing.
+template <class T>
+jf_status plane_sums_static(jf_solver* s, Impl<T>& I, const T* U, int axis, double* out) {
+  const jf::Params<T>& P = I.P;
+  const int np = P.n[axis];
+  if (np > JF_STATIC_MAX_PLANES)
+    return fail(s, JF_EINVAL, "jf_plane_sums_static: more than JF_STATIC_MAX_PLANES = 1024 planes along this axis "
+                              "(the static scratch array holds 14 x 1024 x 16 partial sums); use jf_plane_sums");
+  double* scratch = nullptr;
+  {
+    const cudaError_t ce = static_scratch_ptr(&scratch);
+    if (ce != cudaSuccess || !scratch) return fail(s, JF_ECUDA, "jf_plane_sums_static: cudaGetSymbolAddress(jf_static_scratch)", ce);
+  }
+  const long long ntang = (long long)P.n[(axis + 1) % 3] * P.n[(axis + 2) % 3];
+  int NB = (int)std::min<long long>(STATS_NB, std::max<long long>(1, std::min<long long>((148LL * 8 + np - 1) / np, (ntang + 1023) / 1024)));
+  const dim3 grid(np, NB);
+  if (axis == 0) jf::plane_sums_kernel<T, 0><<<grid, 256, 0, s->stream>>>(P, U, scratch, NB);
+  else if (axis == 1) jf::plane_sums_kernel<T, 1><<<grid, 256, 0, s->stream>>>(P, U, scratch, NB);
+  else jf::plane_sums_kernel<T, 2><<<grid, 256, 0, s->stream>>>(P, U, scratch, NB);
+  jf::plane_sums_final<<<(jf::NSTAT * np + 127) / 128, 128, 0, s->stream>>>(scratch, out, np, NB);
+  s->launches += 2;
+  JF_CUDA(s, cudaPeekAtLastError());
+  return JF_OK;
+}
+
 template <class T>
 jf_status diag_metrics(jf_solver* s, Impl<T>& I, int axis, double* inv_delta, double* centre, double* i12Xc, double* i24Xf) {
   const int Pn = I.P.P[axis];
@@ -1068,6 +1128,18 @@ jf_status jf_plane_sums(jf_solver* s, const void* U, int axis, double* sums) {
   return JF_DISPATCH(s, plane_sums<double>(s, s->d, (const double*)U, axis, sums), plane_sums<float>(s, s->f, (const float*)U, axis, sums),
                      plane_sums<jf::Dual>(s, s->t, (const jf::Dual*)U, axis, sums));
 }
+
+jf_status jf_plane_sums_static(jf_solver* s, const void* U, int axis, double* sums) {
+  if (!s) return JF_EINVAL;
+  DeviceGuard dev_guard(s);
+  if (!U || !sums || axis < 0 || axis > 2) return fail(s, JF_EINVAL, "jf_plane_sums_static: null pointer or bad axis");
+  if (!aligned16(U)) return fail(s, JF_EALIGN, "jf_plane_sums_static: U not 16-byte aligned");
+  return JF_DISPATCH(s, plane_sums_static<double>(s, s->d, (const double*)U, axis, sums),
+                     plane_sums_static<float>(s, s->f, (const float*)U, axis, sums),
+                     plane_sums_static<jf::Dual>(s, s->t, (const jf::Dual*)U, axis, sums));
+}
+
+int jf_plane_sums_static_max_planes(void) { return JF_STATIC_MAX_PLANES; }
 
 jf_status jf_set_tangent_seed(jf_solver* s, double dA, double dkappa) {
   if (!s) return JF_EINVAL;
