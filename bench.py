@@ -296,15 +296,19 @@ def run_ours(args):
     if not args.no_e2e:
         host_in = torch.empty(U.shape, dtype=U.dtype, pin_memory=True)
         host_in.copy_(solver.state().cpu() if args.dtype == "f64t" else torch.as_tensor(case.U0, dtype=U.dtype))
-        host_out = [torch.empty(U.shape, dtype=U.dtype, pin_memory=True) for _ in range(2)]
-        bufs = [U, torch.empty_like(U)]
+        # three device buffers: a buffer is busy for upload + kernels + download (13-16 + 7 + 13-16 ms at 256^3), so with two
+        # of them a job takes half of that (19 ms: measured in round 1-2); with three the copies run back to back and the
+        # PCIe link, both directions at once (measured: 15.7 ms for 719 MB each way), is the limit
+        NBUF = 3
+        host_out = [torch.empty(U.shape, dtype=U.dtype, pin_memory=True) for _ in range(NBUF)]
+        bufs = [U] + [torch.empty_like(U) for _ in range(NBUF - 1)]
         cur = torch.cuda.current_stream(dev)
         s_in, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
 
         def pipeline(njobs):
-            d2h_done = [None, None]
+            d2h_done = [None] * NBUF
             for i in range(njobs):
-                b = i & 1
+                b = i % NBUF
                 with torch.cuda.stream(s_in):
                     if d2h_done[b] is not None:
                         s_in.wait_event(d2h_done[b])           # the buffer's previous result has left the device
@@ -322,7 +326,7 @@ def run_ours(args):
                     cur.wait_event(ev)
 
         Ke = K
-        pipeline(2)
+        pipeline(NBUF)
         barrier()
         t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
         t0.record()
@@ -331,7 +335,7 @@ def run_ours(args):
         barrier()
         ms_e2e = t0.elapsed_time(t1)
         e2e = (ms_e2e, Ke)
-        e2e_finite = bool(torch.isfinite(host_out[(Ke - 1) & 1]).all().item())
+        e2e_finite = bool(torch.isfinite(host_out[(Ke - 1) % NBUF]).all().item())
 
     # --- the other lines of configs[4] (N = 1, default workload only): 384^3 and 512^3 fp64, 512^3 fp32
     sweep = None
@@ -442,7 +446,7 @@ def run_ours(args):
     if e2e:
         line["e2e"] = {"value": job_throughput(cells, e2e[1], world, e2e[0]), "unit": UNIT,
                        "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes, "ms_per_step": e2e[0] / e2e[1],
-                       "pipeline": "double-buffered: H2D of job i+1 and D2H of job i-1 overlap the kernels of job i", "finite": e2e_finite}
+                       "pipeline": "three device buffers: H2D of job i+1 and D2H of job i-1 overlap the kernels of job i; bound by the PCIe link (both directions at once)", "finite": e2e_finite}
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: one RK3 step of the SAME input on the host cores (the oracle as it stands)
         nb = min(n, 256)
