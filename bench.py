@@ -411,6 +411,7 @@ def run_ours(args):
             pk = peak_flops if ln["dtype"] == args.dtype else alu_peak(jf, ln["dtype"], local)[1]
             tr = t_roof_ms(sfm["step"], ln["cells"], ln["dtype"], pk, hbm)
             ln["roofline_step_frac"] = tr / ln["ms_per_step"]
+            ln["roofline_step_frac_at_run_clock"] = (tr / ln["ms_per_step"] * peak_mhz / ln["sm_mhz"]) if (peak_mhz and ln.get("sm_mhz")) else None
             ln["peak_tflops"] = pk / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

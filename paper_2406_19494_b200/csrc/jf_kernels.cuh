@@ -304,6 +304,15 @@ struct alignas(sizeof(T) >= 8 ? 16 : 2 * sizeof(T)) Pair2 { T a, b; };
 #define JF_GM_TY 8
 #endif
 constexpr int GM_TX = 32, GM_TY = JF_GM_TY, GM_SX = GM_TX + 4, GM_SY = GM_TY + 4, GM_RIM = GM_SX * GM_SY - GM_TX * GM_TY;
+// store of a gradient value: write-once data that is not read again before two more passes over the field
+// (JF_GRAD_STCS: as a streaming store)
+template <class T> __device__ __forceinline__ void gst(T* p, T v) {
+#ifdef JF_GRAD_STCS
+  st_cs(p, v);
+#else
+  *p = v;
+#endif
+}
 template <class T>
 __global__ void __launch_bounds__(GM_TX * GM_TY, sizeof(T) > 8 ? JF_GM_MINB_DUAL : JF_GM_MINB)
 gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz) {
@@ -378,8 +387,8 @@ gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz)
           d[c] = (T(8) * (r[1] - r[-1]) - (r[2] - r[-2])) * scx;
         }
         dxu = d[0];
-        (G + (long long)1 * P.vol)[op] = d[1];
-        (G + (long long)2 * P.vol)[op] = d[2];
+        gst((G + (long long)1 * P.vol) + op, d[1]);
+        gst((G + (long long)2 * P.vol) + op, d[2]);
       }
       if (dy_ok) {
         T d[3];
@@ -389,10 +398,10 @@ gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz)
           d[c] = (T(8) * (r[GM_SX] - r[-GM_SX]) - (r[2 * GM_SX] - r[-2 * GM_SX])) * scy;
         }
         dyv = d[1];
-        (G + (long long)3 * P.vol)[op] = d[0];
-        (G + (long long)5 * P.vol)[op] = d[2];
+        gst((G + (long long)3 * P.vol) + op, d[0]);
+        gst((G + (long long)5 * P.vol) + op, d[2]);
       }
-      if (dx_ok && dy_ok) (G + (long long)8 * P.vol)[op] = dxu + dyv;
+      if (dx_ok && dy_ok) gst((G + (long long)8 * P.vol) + op, dxu + dyv);
     }
     const int pzc = p - 2;                     // plane whose z derivative is complete now
     if (own && pzc >= k0 && pzc < k1 && pzc >= NH && pzc < P.n[2] + NH && p - 4 >= pstart) {
@@ -401,10 +410,10 @@ gradient_kernel(Params<T> P, const T* __restrict__ U, T* __restrict__ G, int Lz)
 #pragma unroll
       for (int c = 0; c < 3; ++c) d[c] = (T(8) * (q[3][c] - q[1][c]) - (q[4][c] - q[0][c])) * scz;
       const unsigned oz = op - 2u * sz;
-      (G + (long long)6 * P.vol)[oz] = d[0];
-      (G + (long long)7 * P.vol)[oz] = d[1];
-      if (dy_ok) (G + (long long)0 * P.vol)[oz] = (SQ ? sd[b][1][tid] : dq[0][1]) + d[2];
-      if (dx_ok) (G + (long long)4 * P.vol)[oz] = d[2] + (SQ ? sd[b][0][tid] : dq[0][0]);
+      gst((G + (long long)6 * P.vol) + oz, d[0]);
+      gst((G + (long long)7 * P.vol) + oz, d[1]);
+      if (dy_ok) gst((G + (long long)0 * P.vol) + oz, (SQ ? sd[b][1][tid] : dq[0][1]) + d[2]);
+      if (dx_ok) gst((G + (long long)4 * P.vol) + oz, d[2] + (SQ ? sd[b][0][tid] : dq[0][0]));
     }
     if (SQ) { sd[b][0][tid] = dxu; sd[b][1][tid] = dyv; }   // slot p & 1 held plane p-2 until here
     else { dq[0][0] = dq[1][0]; dq[0][1] = dq[1][1]; dq[1][0] = dxu; dq[1][1] = dyv; }

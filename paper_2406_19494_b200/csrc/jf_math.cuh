@@ -121,6 +121,9 @@ template <> __device__ __forceinline__ Dual with_tangent<Dual>(double v, double 
 // kernel, except the stage input U_s of the fused z + RK sweep, which a thread reads again four march steps
 // after it entered the window: the once-only traffic is marked streaming (evict-first) so that those lines
 // survive in the L2 until their second use, which is marked last-use.
+__device__ __forceinline__ void st_cs(double* p, double v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs(float* p, float v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs(Dual* p, Dual v) { __stcs(reinterpret_cast<double2*>(p), make_double2(v.v, v.d)); }
 #ifdef JF_L2HINTS
 __device__ __forceinline__ double ld_stream(const double* p) { return __ldcs(p); }
 __device__ __forceinline__ float ld_stream(const float* p) { return __ldcs(p); }
