@@ -167,8 +167,9 @@ jf_status jf_dev_time(jf_solver *s, int set, double *dt_host, double *t_host);
  *
  * Environment variables read once, at jf_create (tuning / A-B measurements; none changes a result beyond round-off):
  *   JF_GRAPH=0      plain launches instead of the CUDA-graph replay
- *   JF_GRAD_TMA=1   TMA-staged centre-gradient pass (cp.async.bulk.tensor + mbarrier ring; fp64, even nx): 6 % faster at
- *                   256^3, 22 % slower at 512^3, hence not the default (profiles/r2_tma_sass.md)
+ *   JF_GRAD_TMA=0|1 centre-gradient pass with plain loads | TMA-staged (cp.async.bulk.tensor + mbarrier ring; fp64, even nx
+ *                   only).  Default: TMA for fields of at most 40 M padded cells per variable, where it is 6-8 % faster;
+ *                   plain loads above (at 448^3 and more TMA is 15-22 % slower; profiles/r2_tma_sass.md)
  *   JF_YZ_PC=1      producer / consumer form of the y / z sweeps (fp64, viscous, fourth-order flux): 20 % slower, kept as a
  *                   measured variant (profiles/r2_experiments.md) */
 

@@ -873,11 +873,13 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
     const size_t esz = elem_size(dtype);
     bool ok = dtype == JF_F64 && ((size_t)(g->nx + 6) * esz) % 16 == 0 && encode_tiled_fn() != nullptr;
     const char* e = std::getenv("JF_GRAD_TMA");
-#ifdef JF_GRAD_TMA_DEFAULT
-    bool want = JF_GRAD_TMA_DEFAULT != 0;
-#else
-    bool want = false;
+    // Default by size: the TMA-staged pass is 6-8 % faster than the plain-load pass up to 320^3, equal at 384^3 and
+    // 15 % slower at 448^3 and above (profiles/r2_tma_sass.md), so it is used for fields of at most JF_GRAD_TMA_MAX_CELLS
+    // padded cells per variable (40 M: up to ~335^3).
+#ifndef JF_GRAD_TMA_MAX_CELLS
+#define JF_GRAD_TMA_MAX_CELLS 40000000.0
 #endif
+    bool want = (double)(g->nx + 6) * (double)(g->ny + 6) * (double)(g->nz + 6) <= JF_GRAD_TMA_MAX_CELLS;
     if (e) want = std::atoi(e) != 0;
     s->grad_tma = ok && want;
     if (s->grad_tma) {
