@@ -170,6 +170,8 @@ jf_status jf_dev_time(jf_solver *s, int set, double *dt_host, double *t_host);
  *   JF_GRAD_TMA=0|1 centre-gradient pass with plain loads | TMA-staged (cp.async.bulk.tensor + mbarrier ring; fp64, even nx
  *                   only).  Default: TMA for fields of at most 40 M padded cells per variable, where it is 6-8 % faster;
  *                   plain loads above (at 448^3 and more TMA is 15-22 % slower; profiles/r2_tma_sass.md)
+ *   JF_F32X2=1      fp32 solvers: y / z sweeps with two columns per thread on packed FP32x2 arithmetic (FFMA2): 2-4 % faster on
+ *                   the periodic boxes, slower on the channel, hence not the default (profiles/r2_experiments.md)
  *   JF_YZ_PC=1      producer / consumer form of the y / z sweeps (fp64, viscous, fourth-order flux): 20 % slower, kept as a
  *                   measured variant (profiles/r2_experiments.md) */
 

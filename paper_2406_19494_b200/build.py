@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libjf.so")
 SOURCES = [os.path.join(HERE, "csrc", "jf_api.cu")]
-DEPS = SOURCES + [os.path.join(HERE, "csrc", f) for f in ("jf_kernels.cuh", "jf_math.cuh", "jf_dual.cuh", "jf_tma.cuh", "jf_pc.cuh")] + [
+DEPS = SOURCES + [os.path.join(HERE, "csrc", f) for f in ("jf_kernels.cuh", "jf_math.cuh", "jf_dual.cuh", "jf_tma.cuh", "jf_pc.cuh", "jf_f32x2.cuh")] + [
     os.path.join(ROOT, "include", "jf.h"), os.path.abspath(__file__)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-cudart", "shared"]

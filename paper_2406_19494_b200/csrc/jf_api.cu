@@ -13,6 +13,7 @@
 #include "jf_kernels.cuh"
 #include "jf_tma.cuh"
 #include "jf_pc.cuh"
+#include "jf_f32x2.cuh"
 #include <type_traits>
 #include <cstdlib>
 #include <unordered_map>
@@ -187,6 +188,8 @@ struct jf_solver {
   char* ws = nullptr;
   // TMA-staged gradient pass (jf_tma.cuh): tensor maps per state-array base address (U, stage buffers A, B, ...)
   bool grad_tma = false;
+  bool f32x2 = false;            // fp32 solver: marching sweeps with two columns per thread on packed FP32x2 arithmetic (jf_f32x2.cuh)
+  int seg_len2[3] = {0, 0, 0};   // their segment lengths (half as many warps per layer)
   bool yz_pc = false;            // producer / consumer form of the marching sweeps (jf_pc.cuh; fp64, viscous, fourth order)
   std::unordered_map<const void*, CUtensorMap> maps;
   // CUDA graphs of one RK3 step (the 15 launches), one per state-array address, captured on first use on a private
@@ -574,6 +577,29 @@ jf_status launch_rhs_t(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RKA
       return JF_OK;
     }
   }
+  if constexpr (std::is_same<T, float>::value) {
+    if (s->f32x2) {
+      const size_t sh2 = jf::yz2_smem_bytes<VISC, ORD>();
+      const dim3 blk2(jf::YZ_TX, jf::YZ_TY);
+      auto rows = [](int n) { return ((n + 1) / 2 + jf::YZ_TY - 1) / jf::YZ_TY; };   // blocks over pairs of columns
+      {
+        Timed t(s, K_SWEEP_Y);
+        const int L = s->seg_len2[1];
+        dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, rows(P.n[2]), (P.n[1] + L - 1) / L);
+        jf::sweep_yz2_kernel<1, VISC, 0, ORD><<<grid, blk2, sh2, s->stream>>>(P, U, G, R, none, L);
+      }
+      {
+        Timed t(s, K_SWEEP_Z);
+        const int L = s->seg_len2[2];
+        dim3 grid((P.n[0] + jf::YZ_TX - 1) / jf::YZ_TX, rows(P.n[1]), (P.n[2] + L - 1) / L);
+        if (rk) jf::sweep_yz2_kernel<2, VISC, 2, ORD><<<grid, blk2, sh2, s->stream>>>(P, U, G, R, *rk, L);
+        else jf::sweep_yz2_kernel<2, VISC, 1, ORD><<<grid, blk2, sh2, s->stream>>>(P, U, G, R, none, L);
+      }
+      s->launches += 3;
+      JF_CUDA(s, cudaPeekAtLastError());
+      return JF_OK;
+    }
+  }
   const size_t sh = jf::yz_smem_bytes<T, VISC, ORD>();
   const dim3 blk(jf::YZ_TX, jf::YZ_TY);
   {
@@ -622,6 +648,15 @@ jf_status launch_rhs_o6(jf_solver* s, Impl<T>& I, const T* U, T* R, const jf::RK
 template <>
 jf_status launch_rhs_o6<jf::Dual>(jf_solver* s, Impl<jf::Dual>&, const jf::Dual*, jf::Dual*, const jf::RKArgs<jf::Dual>*) {
   return fail(s, JF_EINVAL, "sixth-order dissipative flux: not built for the tangent type");
+}
+
+template <bool VISC, int ORD>
+cudaError_t opt_in_smem_yz2() {
+  const int sh = (int)jf::yz2_smem_bytes<VISC, ORD>();
+  cudaError_t e = cudaFuncSetAttribute((const void*)jf::sweep_yz2_kernel<1, VISC, 0, ORD>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)jf::sweep_yz2_kernel<2, VISC, 1, ORD>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)jf::sweep_yz2_kernel<2, VISC, 2, ORD>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh);
+  return e;
 }
 
 template <class T>
@@ -908,6 +943,21 @@ jf_status jf_create(jf_solver** out, const jf_grid* g, jf_dtype dtype, double ga
   auto cdiv = [](int a, int b) { return (long long)((a + b - 1) / b); };
   s->seg_len[1] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[2], jf::YZ_TY) * jf::YZ_TY, n[1]);
   s->seg_len[2] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv(n[1], jf::YZ_TY) * jf::YZ_TY, n[2]);
+  {
+    bool want = false;
+#ifdef JF_F32X2_DEFAULT
+    want = JF_F32X2_DEFAULT != 0;
+#endif
+    if (const char* e = std::getenv("JF_F32X2")) want = std::atoi(e) != 0;
+    s->f32x2 = want && dtype == JF_F32;
+    if (s->f32x2) {
+      cudaError_t ce = s->viscous ? opt_in_smem_yz2<true, 4>() : opt_in_smem_yz2<false, 4>();
+      if (ce == cudaSuccess && s->viscous) ce = opt_in_smem_yz2<true, 6>();
+      if (ce != cudaSuccess) s->f32x2 = false;
+      s->seg_len2[1] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv((n[2] + 1) / 2, jf::YZ_TY) * jf::YZ_TY, n[1]);
+      s->seg_len2[2] = pick_segment(cdiv(n[0], jf::YZ_TX) * cdiv((n[1] + 1) / 2, jf::YZ_TY) * jf::YZ_TY, n[2]);
+    }
+  }
   *out = s;
   return JF_OK;
 }

@@ -27,8 +27,40 @@ enum { K_EPS4 = 0, K_13_3, K_SIXTH, K_THIRD, K_4_3, K_2_3, K_COUNT };
 #define JF_KVALS {4e-6, 13.0 / 3.0, 1.0 / 6.0, 1.0 / 3.0, 4.0 / 3.0, 2.0 / 3.0}
 static __constant__ double kConstD[K_COUNT] = JF_KVALS;
 
+// ---- packed single precision: two floats per value, arithmetic by the FP32x2 instructions of sm_100 (FFMA2 / FADD2 /
+// FMUL2: two results per issue slot).  The fp32 sweeps are issue-slot bound (ncu: 78-85 % of the issue slots busy, FMA
+// pipe 52 %), so the marching sweeps can run TWO columns per thread on this type (jf_f32x2.cuh).  Every operation rounds
+// exactly as its scalar counterpart: a column's result does not depend on which column it is paired with.
+struct __align__(8) F2 {
+  float x, y;
+  __device__ __forceinline__ F2() {}
+  __device__ __forceinline__ F2(float a, float b) : x(a), y(b) {}
+  __device__ __forceinline__ F2(float v) : x(v), y(v) {}
+  __device__ __forceinline__ F2(double v) : x((float)v), y((float)v) {}
+  __device__ __forceinline__ F2(int v) : x((float)v), y((float)v) {}
+};
+__device__ __forceinline__ unsigned long long f2_pack(F2 a) { unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y)); return r; }
+__device__ __forceinline__ F2 f2_unpack(unsigned long long r) { F2 a; asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r)); return a; }
+__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(f2_pack(a)), "l"(f2_pack(b)), "l"(f2_pack(c)));
+  return f2_unpack(r);
+}
+__device__ __forceinline__ F2 operator+(F2 a, F2 b) { unsigned long long r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(a)), "l"(f2_pack(b))); return f2_unpack(r); }
+__device__ __forceinline__ F2 operator-(F2 a, F2 b) { unsigned long long r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(a)), "l"(f2_pack(b))); return f2_unpack(r); }
+__device__ __forceinline__ F2 operator*(F2 a, F2 b) { unsigned long long r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(a)), "l"(f2_pack(b))); return f2_unpack(r); }
+__device__ __forceinline__ F2 operator-(F2 a) { return F2(-a.x, -a.y); }     // folds into the operand modifiers of FFMA2 / FADD2
+__device__ __forceinline__ F2& operator+=(F2& a, F2 b) { a = a + b; return a; }
+__device__ __forceinline__ F2& operator-=(F2& a, F2 b) { a = a - b; return a; }
+__device__ __forceinline__ F2& operator*=(F2& a, F2 b) { a = a * b; return a; }
+struct Mask2 { bool x, y; };
+
 template <class T> struct Num;
 template <> struct Num<double> {
+  static constexpr bool NARROW = false;      // fp32 exponent range: the WENO weights must not be formed from products of (beta+eps)^2
+  using Mask = bool;
+  static __device__ __forceinline__ bool ge0(double a) { return a >= 0.0; }
+  static __device__ __forceinline__ double sel(bool m, double a, double b) { return m ? a : b; }
 #ifdef JF_NO_KCONST
   template <int I> static __device__ __forceinline__ double K() { constexpr double k[K_COUNT] = JF_KVALS; return k[I]; }
 #else
@@ -58,6 +90,10 @@ template <> struct Num<double> {
   static __device__ __forceinline__ double abs_(double a) { return fabs(a); }
 };
 template <> struct Num<float> {
+  static constexpr bool NARROW = true;
+  using Mask = bool;
+  static __device__ __forceinline__ bool ge0(float a) { return a >= 0.0f; }
+  static __device__ __forceinline__ float sel(bool m, float a, float b) { return m ? a : b; }
   template <int I> static __device__ __forceinline__ float K() { constexpr double k[K_COUNT] = JF_KVALS; return float(k[I]); }
   static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
   // MUFU seeds (rel. error ~2^-22) refined by one Newton step: ~1 ulp, a fraction of the IEEE sequences
@@ -78,9 +114,39 @@ template <> struct Num<float> {
   static __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
 };
 
+template <> struct Num<F2> {
+  static constexpr bool NARROW = true;
+  using Mask = Mask2;
+  template <int I> static __device__ __forceinline__ F2 K() { constexpr double k[K_COUNT] = JF_KVALS; return F2(float(k[I])); }
+  static __device__ __forceinline__ F2 fma_(F2 a, F2 b, F2 c) { return f2_fma(a, b, c); }
+  static __device__ __forceinline__ F2 rcp(F2 a) {        // as Num<float>::rcp, per component
+    F2 x;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x.x) : "f"(a.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x.y) : "f"(a.y));
+    return f2_fma(x, f2_fma(-a, x, F2(1.0f)), x);
+  }
+  static __device__ __forceinline__ F2 rsqrt_(F2 a) {
+    F2 y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y.x) : "f"(a.x));
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y.y) : "f"(a.y));
+    F2 e = f2_fma(-(a * y), y, F2(1.0f));
+    return f2_fma(y, F2(0.5f) * e, y);
+  }
+  static __device__ __forceinline__ F2 sqrt_(F2 a) { return a * rsqrt_(a); }
+  static __device__ __forceinline__ F2 min_(F2 a, F2 b) { return F2(fminf(a.x, b.x), fminf(a.y, b.y)); }
+  static __device__ __forceinline__ F2 max_(F2 a, F2 b) { return F2(fmaxf(a.x, b.x), fmaxf(a.y, b.y)); }
+  static __device__ __forceinline__ F2 abs_(F2 a) { return F2(fabsf(a.x), fabsf(a.y)); }
+  static __device__ __forceinline__ Mask2 ge0(F2 a) { return Mask2{a.x >= 0.0f, a.y >= 0.0f}; }
+  static __device__ __forceinline__ F2 sel(Mask2 m, F2 a, F2 b) { return F2(m.x ? a.x : b.x, m.y ? a.y : b.y); }
+};
+
 // tangent scalar: value part by the same formulas as Num<double>, tangent by the chain rule
 template <> struct Num<Dual> {
   using D = Num<double>;
+  static constexpr bool NARROW = false;
+  using Mask = bool;
+  static __device__ __forceinline__ bool ge0(Dual a) { return a.v >= 0.0; }
+  static __device__ __forceinline__ Dual sel(bool m, Dual a, Dual b) { return m ? a : b; }
   template <int I> static __device__ __forceinline__ Dual K() { return Dual(kConstD[I]); }
   static __device__ __forceinline__ Dual fma_(Dual a, Dual b, Dual c) {
     return Dual(fma(a.v, b.v, c.v), fma(a.v, b.d, fma(a.d, b.v, c.d)));
@@ -197,7 +263,7 @@ __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp
   T e1 = N::fma_(c133 * A1, A1, N::fma_(b1, b1, eps4));
   T e2 = N::fma_(c133 * A2, A2, N::fma_(b2, b2, eps4));
   T E12, E02, E01;
-  if (sizeof(T) == 4) {
+  if (N::NARROW) {
     // fp32: the pair products e_k e_l ~ beta^4 ~ (jump)^8 leave the exponent range once a primitive jumps by ~1e4
     // (SI pressures with a mild shock).  Dividing all three products by e_0 e_1 e_2 leaves the weights unchanged
     // and gives (E12, E02, E01) = (1/e_0, 1/e_1, 1/e_2): three reciprocals, every factor within range.
@@ -243,11 +309,11 @@ __device__ __forceinline__ void hllc_rot(const Gas<T>& gas, const T L[5], const 
   T mL = L[0] * (SL - L[1]), mR = R[0] * (SR - R[1]);
   T Ss = (R[4] - L[4] + L[1] * mL - R[1] * mR) * N::rcp(mL - mR);
   // side selected by sign(S*)  (S* == 0: both star fluxes are mathematically equal)
-  bool left = Ss >= T(0);
-  T rho = left ? L[0] : R[0], vn = left ? L[1] : R[1], v1 = left ? L[2] : R[2], v2 = left ? L[3] : R[3];
-  T p = left ? L[4] : R[4], hq = left ? hL : hR, SK = left ? SL : SR, m = left ? mL : mR;
-  T ri = left ? riL : riR;
-  T Sc = left ? N::min_(SL, T(0)) : N::max_(SR, T(0));  // min(S_L,0) / max(S_R,0)
+  const typename N::Mask left = N::ge0(Ss);
+  T rho = N::sel(left, L[0], R[0]), vn = N::sel(left, L[1], R[1]), v1 = N::sel(left, L[2], R[2]), v2 = N::sel(left, L[3], R[3]);
+  T p = N::sel(left, L[4], R[4]), hq = N::sel(left, hL, hR), SK = N::sel(left, SL, SR), m = N::sel(left, mL, mR);
+  T ri = N::sel(left, riL, riR);
+  T Sc = N::sel(left, N::min_(SL, T(0)), N::max_(SR, T(0)));  // min(S_L,0) / max(S_R,0)
   T E = N::fma_(rho, hq, p * gas.inv_gm1);
   T mn = rho * vn;
   T dinv = N::rcp(SK - Ss);
