@@ -578,6 +578,16 @@ def test_device_resident_dt_equals_the_host_loop(jf, ora, name):
     assert np.all(metric_P(Ud.cpu().numpy(), Uo) <= TOL["f64"])
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64t"])
+def test_device_resident_dt_other_dtypes(jf, dtype):
+    # the same equality (dt sequence and state, bit for bit) for the fp32 and the tangent solver
+    c = cases.channel(24, 16, 16, n_steps=8)
+    Uh, dth = jf.run_case(c, dtype)
+    Ud, dtd = jf.run_case(c, dtype, device_dt=True)
+    assert dth == dtd and len(dth) == 8
+    assert Uh.cpu().numpy().tobytes() == Ud.cpu().numpy().tobytes()
+
+
 def test_device_resident_dt_flags_bad_state(jf):
     c = cases.random_admissible(n=(12, 10, 8), seed=1)
     s = jf.Solver(c)
