@@ -8,7 +8,8 @@
  *   :54-62) face fluxes with per-cell widths, plus sources                   Eq. 6, :64-69
  *   convective face flux: WENO-type reconstruction + approximate Riemann solver (:72) —
  *   here WENO5-JS on primitive variables + HLLC (:88); dissipative flux: central finite
- *   differences (:72) — here 4th order, Sutherland viscosity (:108), Fourier heat flux (:62)
+ *   differences (:72) — here 4th order (6th order, the paper's DNS, :90, by jf_set_visc_order),
+ *   Sutherland viscosity (:108), Fourier heat flux (:62)
  *   time integration: explicit TVD Runge-Kutta (:72) — here SSP-RK3
  *   arrays carry Nh = 3 halo cells per side, shape [N+2Nh]^3 (:80); boundary conditions are
  *   imposed by assigning the halo cells (:100): periodic, zero-gradient, Dirichlet, no-slip wall
@@ -26,7 +27,10 @@
  *       index ((q*(nz+6) + k+3)*(ny+6) + j+3)*(nx+6) + i+3,  q in {rho, rho u, rho v, rho w, E},
  *     x fastest; base address 16-byte aligned (JF_EALIGN otherwise).
  *   - Every launch goes to the cuda_stream given to jf_create (a cudaStream_t passed as
- *     void*; NULL = default stream).  Only jf_cfl_dt and jf_diag_* synchronise that stream.
+ *     void*; NULL = default stream).  Only jf_cfl_dt, jf_dev_time, jf_set_visc_order, jf_set_tangent_seed and
+ *     jf_diag_* synchronise that stream.
+ *   - A solver belongs to the CUDA device that was current at jf_create (its workspace must live there: JF_EINVAL
+ *     otherwise); every call makes that device current for its duration and restores the caller's.
  *   - One jf_solver per host thread / stream (thread-compatible, not thread-safe).
  *   - There is no CPU fallback: without a CUDA device every compute call fails with JF_ECUDA.
  */
